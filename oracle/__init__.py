@@ -1,0 +1,118 @@
+"""TEST INFRASTRUCTURE -- float64 CPU oracle (ctypes wrapper around oracle/gridder_oracle.cpp).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  The product (paper_1605_07023_b200) never does and has no CPU fallback.
+
+What it computes and which passage each step follows is documented in gridder_oracle.cpp; the
+readings of the paper are DESIGN.md R1-R24.  "Parity unpinned": physical tap positions inside the
+table (see gridder_oracle.cpp header).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gridder_oracle.cpp")
+_LIB = os.path.join(_HERE, "libgridder_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ -O3 -fopenmp (no CUDA headers, separate translation unit)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O3", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+               "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        c_int, c_ll, vp = ctypes.c_int, ctypes.c_longlong, ctypes.c_void_p
+        lib.oracle_quantise.argtypes = [c_int] * 4 + [c_ll] + [vp] * 7
+        lib.oracle_quantise.restype = c_int
+        lib.oracle_grid.argtypes = [c_int] * 5 + [c_ll] + [vp] * 5 + [c_int] * 3 + [vp]
+        lib.oracle_grid.restype = c_int
+        lib.oracle_degrid.argtypes = [c_int] * 5 + [c_ll] + [vp] * 5
+        lib.oracle_degrid.restype = c_int
+        lib.oracle_max_threads.restype = c_int
+        _lib = lib
+    return _lib
+
+
+def _f32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if shape is not None:
+        assert a.shape == shape, (a.shape, shape)
+    return a
+
+
+def _c64(a):
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.complex64, a.dtype
+    return a
+
+
+def max_threads() -> int:
+    return int(_load().oracle_max_threads())
+
+
+def quantise(grid_size, support, oversample, n_wplanes, uvw):
+    """Q and W of DESIGN.md R4/R5 -> dict of int32 arrays i0, j0, su, sv, wp and uint8 valid."""
+    lib = _load()
+    uvw = _f32(uvw)
+    n = uvw.shape[0]
+    out = {k: np.empty(n, dtype=np.int32) for k in ("i0", "j0", "su", "sv", "wp")}
+    out["valid"] = np.empty(n, dtype=np.uint8)
+    rc = lib.oracle_quantise(grid_size, support, oversample, n_wplanes, n, uvw.ctypes.data,
+                             *(out[k].ctypes.data for k in ("i0", "j0", "su", "sv", "wp", "valid")))
+    if rc != 0:
+        raise ValueError("oracle_quantise: invalid arguments")
+    return out
+
+
+def grid(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis, weights, kernel,
+         rows=None, n_threads=0, out=None, return_valid=False):
+    """complex128 grid [rows][N][P] (+= into ``out`` if given).  rows=(lo, hi) restricts to a row band."""
+    lib = _load()
+    uvw = _f32(uvw)
+    n = uvw.shape[0]
+    vis = _c64(vis).reshape(n, n_pol)
+    weights = _f32(weights, (n,))
+    kernel = _c64(kernel)
+    assert kernel.shape == (n_wplanes, oversample, support), kernel.shape
+    lo, hi = (0, grid_size) if rows is None else rows
+    if out is None:
+        out = np.zeros((hi - lo, grid_size, n_pol), dtype=np.complex128)
+    assert out.shape == (hi - lo, grid_size, n_pol) and out.dtype == np.complex128
+    assert out.flags.c_contiguous
+    nv = ctypes.c_longlong(0)
+    rc = lib.oracle_grid(grid_size, support, oversample, n_wplanes, n_pol, n, uvw.ctypes.data,
+                         vis.ctypes.data, weights.ctypes.data, kernel.ctypes.data, out.ctypes.data,
+                         lo, hi, n_threads, ctypes.addressof(nv))
+    if rc != 0:
+        raise ValueError("oracle_grid: invalid arguments")
+    return (out, int(nv.value)) if return_valid else out
+
+
+def degrid(grid_size, support, oversample, n_wplanes, n_pol, uvw, weights, kernel, grid_in):
+    """Adjoint of grid() (pin P7 only): complex128 [n_vis][P]."""
+    lib = _load()
+    uvw = _f32(uvw)
+    n = uvw.shape[0]
+    weights = _f32(weights, (n,))
+    kernel = _c64(kernel)
+    g = np.ascontiguousarray(grid_in, dtype=np.complex128)
+    assert g.shape == (grid_size, grid_size, n_pol)
+    out = np.empty((n, n_pol), dtype=np.complex128)
+    rc = lib.oracle_degrid(grid_size, support, oversample, n_wplanes, n_pol, n, uvw.ctypes.data,
+                           weights.ctypes.data, kernel.ctypes.data, g.ctypes.data, out.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_degrid: invalid arguments")
+    return out

@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- gridding throughput on seeded synthetic workloads (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1] [--impl ours|reference]
+
+One "step" = one whole grid_execute (quantise pass a1 + gridding kernel a2-a9) over the full workload
+of the named config.  `value` = grid-point updates/s = n_valid * S^2 * P * K / t (padding cells not
+counted), inputs resident in HBM; `e2e` = the same with the host->device copy of all inputs and a
+device->host read of the grid inside the timed region.  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+# FP32 FMA roofline of one B200: 148 SMs x 128 FP32 lanes x 2 flops x 1.965 GHz (guide's unit counts
+# and clocks.max.sm).  8 flops per grid-point update.
+PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+FLOPS_PER_UPDATE = 8
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--tuning", default="", help="e.g. cu=2,cv=2,threads_per_cta=256")
+    return ap.parse_args()
+
+
+def metric_name():
+    return "grid-point updates/s (x pols)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def oracle_sample(wl, stride):
+    """Every `stride`-th baseline of the workload (bounded sample for the CPU legs)."""
+    c = wl.cfg
+    per_bl = c.n_times * c.n_chan
+    sel = np.arange(0, c.n_baselines, stride)
+    idx = (sel[:, None] * per_bl + np.arange(per_bl)[None, :]).ravel()
+    return wl.uvw[idx], wl.vis[idx], wl.weights[idx], len(sel)
+
+
+def time_oracle(wl, stride, reps=1):
+    import oracle
+    c = wl.cfg
+    uvw, vis, wts, n_bl = oracle_sample(wl, stride)
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        _, n_valid = oracle.grid(c.grid_size, c.support, c.oversample, c.n_wplanes, c.n_pol, uvw, vis, wts,
+                                 wl.kernel, return_valid=True)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    updates = n_valid * c.support ** 2 * c.n_pol
+    return updates / best, best, updates, n_bl, oracle.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the float64 oracle, as it stands, on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1605_07023_b200 import synth
+    import oracle
+    oracle.build()
+    cfg = synth.get_config(args.config)
+    wl = synth.make_workload(cfg)
+    stride = 8 if cfg.n_baselines >= 64 else 1
+    for _ in range(args.warmup):
+        time_oracle(wl, stride)
+    t_total, updates = 0.0, 0
+    for _ in range(args.steps):
+        _, dt, upd, n_bl, cores = time_oracle(wl, stride)
+        t_total += dt
+        updates += upd
+    value = updates / t_total
+    sample = f"every {stride}th baseline of {cfg.name} ({n_bl} of {cfg.n_baselines} baselines, {upd:.3e} updates per step)"
+    line = {
+        "impl": "reference", "metric": metric_name(), "value": value, "unit": "updates/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_vis": cfg.n_vis, "grid": cfg.grid_size, "support": cfg.support,
+                   "oversample": cfg.oversample, "n_wplanes": cfg.n_wplanes, "n_pol": cfg.n_pol},
+        "cpu_baseline": {"value": value, "unit": "updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def parse_tuning(text):
+    out = {}
+    for item in filter(None, text.split(",")):
+        k, v = item.split("=")
+        out[k.strip()] = int(v)
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1605_07023_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gridder has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # Weak scaling: every rank grids its own full workload (same recipe, seed + rank) onto its own
+    # grid -- independent problems like the paper's W-stacking slices; no collective.
+    cfg = synth.get_config(args.config)
+    if rank > 0:
+        from dataclasses import replace
+        cfg = replace(cfg, seed=cfg.seed + 1000 * rank)
+    wl = synth.make_workload(cfg)
+    N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
+
+    h_uvw = torch.from_numpy(wl.uvw).pin_memory()
+    h_vis = torch.from_numpy(wl.vis).pin_memory()
+    h_wts = torch.from_numpy(wl.weights).pin_memory()
+    d_uvw, d_vis, d_wts = h_uvw.to(dev), h_vis.to(dev), h_wts.to(dev)
+    d_kern = torch.from_numpy(wl.kernel).to(dev)
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(cfg.n_vis)
+    plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    tuning = parse_tuning(args.tuning)
+    if tuning:
+        plan.set_tuning(**tuning)
+    plan.allocate_workspace(dev)
+    info = plan.info()
+
+    # number of valid samples (for the metric) from the library's own quantise pass
+    q = plan.quantise(d_uvw)
+    n_valid = int(q[:, 5].sum().item())
+    del q
+    updates_per_step = n_valid * S * S * P
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+    barrier()
+
+    # ---- device-resident timing: exactly K steps, CUDA events on the launching stream
+    k_events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                for _ in range(args.steps)]
+    for a, b in k_events:            # force creation of the underlying cudaEvent_t
+        a.record(stream)
+        b.record(stream)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches = 0
+    ev0.record(stream)
+    for k in range(args.steps):
+        plan.set_kernel_events(*k_events[k])
+        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        launches += plan.last_launches()
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    plan.set_kernel_events(None, None)
+    elapsed_ms = ev0.elapsed_time(ev1)
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in k_events]))
+
+    # ---- end to end: pinned host inputs -> device, execute, grid -> pinned host, every step
+    e2e = None
+    if not args.no_e2e:
+        h_grid = torch.empty((N, N, P), dtype=torch.complex64).pin_memory()
+        e_steps = max(3, min(args.steps, 10))
+        h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4
+        d2h = h_grid.numel() * 8
+        for _ in range(2):
+            d_uvw.copy_(h_uvw, non_blocking=True)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(e_steps):
+            d_uvw.copy_(h_uvw, non_blocking=True)
+            d_vis.copy_(h_vis, non_blocking=True)
+            d_wts.copy_(h_wts, non_blocking=True)
+            plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+            h_grid.copy_(grid, non_blocking=True)
+        e1.record(stream)
+        barrier()
+        e2e_ms = e0.elapsed_time(e1)
+        e2e = {"ms": e2e_ms, "steps": e_steps, "h2d": h2d, "d2h": d2h}
+
+    t = torch.tensor([elapsed_ms, e2e["ms"] / e2e["steps"] if e2e else 0.0, kernel_ms], device=dev, dtype=torch.float64)
+    tot = torch.tensor([float(updates_per_step)], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    elapsed_ms, e2e_step_ms, kernel_ms = (float(x) for x in t.tolist())
+    total_updates_per_step = float(tot.item())
+
+    if rank == 0:
+        value = total_updates_per_step * args.steps / (elapsed_ms * 1e-3)
+        achieved = updates_per_step * FLOPS_PER_UPDATE / (kernel_ms * 1e-3) / 1e12
+        line = {
+            "metric": metric_name(), "value": value, "unit": "updates/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": elapsed_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "n_vis": cfg.n_vis, "n_valid": n_valid, "grid": N, "support": S,
+                       "oversample": O, "n_wplanes": W, "n_pol": P, "updates_per_step": updates_per_step,
+                       "l2": "inputs (%.2f GB per step) exceed the 126 MB L2; no explicit flush" %
+                             ((h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4) / 1e9),
+                       "tuning": info},
+            "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
+                         "frac": achieved / PEAK_FP32_TFLOPS, "traffic": None,
+                         "kernel": "grid_coarsened_kernel", "kernel_ms": kernel_ms,
+                         "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (derived; DESIGN.md)"},
+            "clocks": clocks, "gpu_launches": launches,
+        }
+        if e2e:
+            line["e2e"] = {"value": total_updates_per_step / (e2e_step_ms * 1e-3), "unit": "updates/s",
+                           "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                           "ms_per_step": e2e_step_ms}
+        if not args.no_cpu_baseline and world >= 1:
+            stride = 4 if cfg.n_baselines >= 64 else 1
+            v, dt, upd, n_bl, cores = time_oracle(wl, stride)
+            line["cpu_baseline"] = {"value": v, "unit": "updates/s", "cores": cores, "kind": "oracle",
+                                    "sample": f"every {stride}th baseline of {cfg.name} ({n_bl} baselines, "
+                                              f"{upd:.3e} updates, {dt:.1f} s)"}
+        print(json.dumps(line), flush=True)
+    plan.destroy()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

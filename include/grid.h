@@ -1,0 +1,113 @@
+/* grid.h -- C ABI of the B200 convolutional gridder (libgridb200.so).
+ *
+ * The operation (section 2.2): "each visibility sample is treated as a Dirac delta,
+ * convolved with some function, and then sampled onto the grid"; the gridding convolution function
+ * (GCF) is read from a precomputed oversampled table selected per sample by "the
+ * integer grid coordinates, the sub-grid coordinates for indexing the GCF, the w plane index"
+ * (section 4); the GCF is separable, G_ij = Gu_i * Gv_j, and polarisation-independent
+ * (PAPER.md:97-99, 178).  The two main entry points are the ones BASELINE.json:north_star fixes.
+ * Exact semantics (quantiser, layouts, edge handling): DESIGN.md "Readings" R1-R24.
+ *
+ * Conventions
+ *   - Every array argument is a DEVICE pointer owned by the caller, 16-byte aligned, unless it says
+ *     HOST.  The library allocates no device memory; scratch space is the caller's workspace.
+ *   - Return value 0 = success, negative = GRID_ERR_*; grid_last_error() gives a thread-local text.
+ *   - All work is enqueued on `stream`; no call synchronises the host with the device.
+ *   - A plan may be executed repeatedly; calls on one plan must not overlap in time.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails.
+ */
+#ifndef GRIDB200_GRID_H
+#define GRIDB200_GRID_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GRID_OK                 0
+#define GRID_ERR_INVALID_ARG   -1
+#define GRID_ERR_UNSUPPORTED   -2   /* e.g. tap tables + batch buffers exceed shared memory */
+#define GRID_ERR_CUDA          -3
+#define GRID_ERR_STATE         -4   /* set_samples / set_workspace missing or too small */
+
+typedef struct grid_plan grid_plan;           /* opaque, owned by the library */
+typedef struct CUstream_st* grid_stream_t;    /* == cudaStream_t */
+
+/* Create a plan for an N x N grid (BASELINE.json:north_star signature).
+ *   grid_size  N, 1 <= N <= 32767, N >= support
+ *   support    S >= 1, odd or even; footprint is S x S cells
+ *   oversample O >= 1; taps tabulated at 1/O cell
+ *   n_wplanes  >= 1, n_wplanes * oversample <= 65535
+ *   n_pol      1, 2 or 4 complex polarisations per sample
+ * Chooses the coarsening block (Cu x Cv), threads per CTA and batch length from a tuned table
+ * keyed by (S, n_pol).  Returns NULL on error. */
+grid_plan* grid_plan_create(int grid_size, int support, int oversample, int n_wplanes, int n_pol);
+
+/* Number of samples of the next grid_execute calls (the execute signature carries no count).
+ * n_vis >= 0; n_vis == 0 makes grid_execute a no-op (R23). */
+int grid_plan_set_samples(grid_plan* plan, long long n_vis);
+
+/* OPTIONAL performance hint: samples are ordered baseline-major, then time, then channel
+ * (BASELINE.json:configs[0]), n_baselines*n_times*n_channels == n_vis.  It only changes the order in
+ * which a chunk's samples are traversed (the sum is order-independent up to FP32 rounding, pin P11);
+ * never the result beyond that.  Pass zeros to clear. */
+int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_channels);
+
+/* Scratch memory the plan needs for the current n_vis (quantised sample records + counters). */
+size_t grid_plan_workspace_bytes(const grid_plan* plan);
+/* Caller-owned device scratch, >= grid_plan_workspace_bytes(), 256-byte aligned. */
+int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes);
+
+/* Grid all samples:  for every sample n whose S x S footprint lies inside the grid (others, and
+ * samples with non-finite u, v or w, are skipped, R7):
+ *     grid[j0+tj][i0+ti][p] += weights[n] * vis[n][p] * k[wp][sv][tj] * k[wp][su][ti]
+ * with (i0,su) = Q(u_n), (j0,sv) = Q(v_n), wp = W(w_n) (R4, R5), FP32 arithmetic,
+ * FP32 atomic accumulation (order nondeterministic).
+ *   uvw          [n_vis][3] float32: u, v in cells from the centre cell floor(N/2); w in plane units
+ *   vis          [n_vis][n_pol] complex64 (re, im interleaved), polarisation fastest
+ *   weights      [n_vis] float32
+ *   conv_kernel  [n_wplanes][oversample][support] complex64 separable taps (same table for u and v)
+ *   grid         [N][N][n_pol] complex64, row = v, column = u; ACCUMULATED INTO, never zeroed
+ * Steps: a1 quantise pass, then the gridding kernel (a2-a9). */
+int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                 const float* conv_kernel, float* grid, grid_stream_t stream);
+
+/* Step a1 alone (the device pass that turns uvw into integer cell, sub-offset and plane index),
+ * unpacked for inspection: out is int32 [n][6] = i0, j0, su, sv, wp, valid (invalid: -1 x5, 0).
+ * Runs the same device function grid_execute uses.  n need not equal the plan's n_vis. */
+int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid_stream_t stream);
+
+/* Override the tuned launch configuration (autotuning).  Any argument <= 0 keeps the
+ * current value.  variant: 1 = coarsened register-accumulating kernel (default),
+ * 0 = naive scatter (one atomic per update; diagnostic baseline only).
+ *   cu, cv            coarsening block per thread (u, v), each in {1,2,4,8}, cu*cv*n_pol <= 32
+ *   threads_per_cta   multiple of 32, <= 1024
+ *   batch             samples staged to shared memory per team per step
+ *   chunk             samples a team grids before its final flush (1024)
+ *   ctas_per_sm       persistent CTAs per SM
+ * Returns GRID_ERR_UNSUPPORTED if the combination does not fit (shared memory, registers). */
+int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threads_per_cta,
+                         int batch, int chunk, int ctas_per_sm);
+
+/* HOST out[16]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
+ * chunk, ctas_per_sm, smem_bytes, n_sm, traversal (0 input order, 1 time-inner), 0, 0. */
+int grid_plan_get_info(const grid_plan* plan, int* out);
+
+/* Measurement hook: two caller-owned cudaEvent_t (passed as void*) that the following grid_execute
+ * calls record on `stream` immediately before and after the gridding kernel (steps a2-a9; the
+ * quantise pass a1 lies outside the pair).  NULL, NULL clears.  Nothing is synchronised. */
+int grid_plan_set_kernel_events(grid_plan* plan, void* ev_start, void* ev_stop);
+
+/* Kernel launches enqueued by the last grid_execute on this plan (for bench.py's gpu_launches). */
+int grid_plan_last_launches(const grid_plan* plan);
+
+void grid_plan_destroy(grid_plan* plan);
+
+/* Thread-local description of the last error in this thread ("" if none). */
+const char* grid_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRIDB200_GRID_H */

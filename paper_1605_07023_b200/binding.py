@@ -1,0 +1,188 @@
+"""Thin ctypes binding over libgridb200.so (include/grid.h).  Argument marshalling only: every step
+of the hot path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+
+There is no CPU fallback: if the shared library is missing, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgridb200.so")
+
+GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STATE = 0, -1, -2, -3, -4
+
+EXPORTS = (
+    "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
+    "grid_plan_set_workspace", "grid_execute", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_get_info", "grid_plan_set_kernel_events", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
+)
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+        "(nvcc, sm_100a).  The gridder has no CPU fallback.")
+
+_lib = ctypes.CDLL(LIB_PATH)
+_vp, _int, _ll, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_size_t
+_lib.grid_plan_create.argtypes = [_int] * 5
+_lib.grid_plan_create.restype = _vp
+_lib.grid_plan_set_samples.argtypes = [_vp, _ll]
+_lib.grid_plan_set_layout.argtypes = [_vp, _int, _int, _int]
+_lib.grid_plan_workspace_bytes.argtypes = [_vp]
+_lib.grid_plan_workspace_bytes.restype = _sz
+_lib.grid_plan_set_workspace.argtypes = [_vp, _vp, _sz]
+_lib.grid_execute.argtypes = [_vp] * 7
+_lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
+_lib.grid_plan_set_tuning.argtypes = [_vp] + [_int] * 7
+_lib.grid_plan_get_info.argtypes = [_vp, _vp]
+_lib.grid_plan_set_kernel_events.argtypes = [_vp, _vp, _vp]
+_lib.grid_plan_last_launches.argtypes = [_vp]
+_lib.grid_plan_destroy.argtypes = [_vp]
+_lib.grid_plan_destroy.restype = None
+_lib.grid_last_error.restype = ctypes.c_char_p
+
+
+class GridError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: error {code}: {_lib.grid_last_error().decode()}")
+
+
+def grid_last_error() -> str:
+    return _lib.grid_last_error().decode()
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != GRID_OK:
+        raise GridError(rc, where)
+
+
+def _ptr(t, dtype, what):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{what}: expected a CUDA torch.Tensor (device pointers only; no CPU fallback)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{what}: expected contiguous {dtype}, got {t.dtype} contiguous={t.is_contiguous()}")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+INFO_FIELDS = ("variant", "cu", "cv", "bin_u", "bin_v", "team_threads", "teams_per_cta",
+               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal")
+
+
+class GridPlan:
+    """Owns a grid_plan* (same names as the C ABI: set_samples, set_layout, set_workspace, execute)."""
+
+    def __init__(self, grid_size, support, oversample, n_wplanes, n_pol):
+        self._h = _lib.grid_plan_create(grid_size, support, oversample, n_wplanes, n_pol)
+        if not self._h:
+            raise GridError(GRID_ERR_INVALID_ARG, "grid_plan_create")
+        self.grid_size, self.support, self.oversample = grid_size, support, oversample
+        self.n_wplanes, self.n_pol = n_wplanes, n_pol
+        self.n_vis = None
+        self._workspace = None
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            _lib.grid_plan_destroy(self._h)
+            self._h = None
+            self._workspace = None
+
+    __del__ = destroy
+
+    def set_samples(self, n_vis: int):
+        _check(_lib.grid_plan_set_samples(self._h, n_vis), "grid_plan_set_samples")
+        self.n_vis = n_vis
+
+    def set_layout(self, n_baselines: int, n_times: int, n_channels: int):
+        _check(_lib.grid_plan_set_layout(self._h, n_baselines, n_times, n_channels), "grid_plan_set_layout")
+
+    def workspace_bytes(self) -> int:
+        return int(_lib.grid_plan_workspace_bytes(self._h))
+
+    def set_workspace(self, tensor):
+        import torch
+        ptr = _ptr(tensor, torch.uint8, "workspace")
+        _check(_lib.grid_plan_set_workspace(self._h, ptr, tensor.numel()), "grid_plan_set_workspace")
+        self._workspace = tensor          # keep the caller's buffer alive
+
+    def allocate_workspace(self, device="cuda"):
+        import torch
+        self.set_workspace(torch.empty(max(self.workspace_bytes(), 256), dtype=torch.uint8, device=device))
+
+    def set_tuning(self, variant=-1, cu=0, cv=0, threads_per_cta=0, batch=0, chunk=0, ctas_per_sm=0):
+        _check(_lib.grid_plan_set_tuning(self._h, variant, cu, cv, threads_per_cta, batch, chunk, ctas_per_sm),
+               "grid_plan_set_tuning")
+
+    def info(self) -> dict:
+        out = (ctypes.c_int * 16)()
+        _check(_lib.grid_plan_get_info(self._h, out), "grid_plan_get_info")
+        return dict(zip(INFO_FIELDS, list(out)))
+
+    def set_kernel_events(self, ev_start=None, ev_stop=None):
+        """torch.cuda.Event pair (enable_timing=True, already created) recorded around the gridding kernel."""
+        a = ev_start.cuda_event if ev_start is not None else None
+        b = ev_stop.cuda_event if ev_stop is not None else None
+        _check(_lib.grid_plan_set_kernel_events(self._h, a, b), "grid_plan_set_kernel_events")
+
+    def last_launches(self) -> int:
+        return int(_lib.grid_plan_last_launches(self._h))
+
+    def execute(self, uvw, vis, weights, conv_kernel, grid, stream=None):
+        """grid += gridded samples (grid_execute).  All arguments are CUDA tensors:
+        uvw float32 [n][3], vis complex64 [n][P], weights float32 [n],
+        conv_kernel complex64 [W][O][S], grid complex64 [N][N][P]."""
+        import torch
+        n = self.n_vis
+        if n is None:
+            raise GridError(GRID_ERR_STATE, "grid_execute (set_samples not called)")
+        if n > 0 and (uvw.numel() != 3 * n or vis.numel() != n * self.n_pol or weights.numel() != n):
+            raise ValueError("array sizes do not match set_samples()")
+        if conv_kernel.numel() != self.n_wplanes * self.oversample * self.support:
+            raise ValueError("conv_kernel must be [n_wplanes][oversample][support]")
+        if grid.numel() != self.grid_size * self.grid_size * self.n_pol:
+            raise ValueError("grid must be [N][N][n_pol]")
+        rc = _lib.grid_execute(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
+                               _ptr(weights, torch.float32, "weights"),
+                               _ptr(conv_kernel, torch.complex64, "conv_kernel"),
+                               _ptr(grid, torch.complex64, "grid"), _stream(stream))
+        _check(rc, "grid_execute")
+
+    def quantise(self, uvw, stream=None):
+        """Step a1 alone -> int32 CUDA tensor [n][6] = i0, j0, su, sv, wp, valid."""
+        import torch
+        n = uvw.shape[0]
+        out = torch.empty((n, 6), dtype=torch.int32, device=uvw.device)
+        _check(_lib.grid_quantise(self._h, _ptr(uvw, torch.float32, "uvw"), n, out.data_ptr(), _stream(stream)),
+               "grid_quantise")
+        return out
+
+
+def grid_visibilities(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis, weights, conv_kernel,
+                      grid=None, layout=None, tuning=None):
+    """One-shot convenience wrapper over the plan calls; returns the (accumulated) grid tensor."""
+    import torch
+    plan = GridPlan(grid_size, support, oversample, n_wplanes, n_pol)
+    try:
+        plan.set_samples(uvw.shape[0])
+        if layout:
+            plan.set_layout(*layout)
+        if tuning:
+            plan.set_tuning(**tuning)
+        plan.allocate_workspace(uvw.device)
+        if grid is None:
+            grid = torch.zeros((grid_size, grid_size, n_pol), dtype=torch.complex64, device=uvw.device)
+        plan.execute(uvw, vis, weights, conv_kernel, grid)
+        torch.cuda.current_stream().synchronize()
+    finally:
+        plan.destroy()
+    return grid

@@ -1,0 +1,341 @@
+// Host side of libgridb200.so: the C ABI of include/grid.h.  Product path only -- no CPU fallback,
+// nothing from oracle/.
+#include "../../include/grid.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "grid_kernel.cuh"
+#include "gridder_common.cuh"
+#include "quantise.cuh"
+
+using namespace gridb200;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+}  // namespace
+
+struct grid_plan {
+    int N, S, O, W, P;
+    long long n_vis;
+    int n_baselines, n_times, n_channels;
+    void* workspace;
+    size_t workspace_bytes;
+    // tuning
+    int variant, cu, cv, threads, batch, chunk, ctas_per_sm;
+    // derived
+    int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
+    int n_sm, max_smem;
+    int last_launches;
+    cudaEvent_t ev_start, ev_stop;
+};
+
+namespace {
+
+typedef void (*kernel_fn)(const GridParams);
+
+template <int CU, int CV, int P>
+kernel_fn pick() { return grid_coarsened_kernel<CU, CV, P>; }
+
+// Instantiated coarsening blocks: near-square shapes only, Cu*Cv*P <= 32 accumulators.
+kernel_fn lookup_kernel(int cu, int cv, int P) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick<a, b, p>();
+    CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 1, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 2, 1) CASE(8, 4, 1)
+    CASE(1, 1, 2) CASE(2, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
+    CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 1, 4) CASE(4, 2, 4)
+#undef CASE
+    return nullptr;
+}
+
+size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec); }
+
+// Derive bins, team shape and shared-memory footprint from the tuning; validate.
+int derive(grid_plan* p) {
+    if (p->variant == 0) {
+        p->bin_u = p->bin_v = p->row_u = p->row_v = p->S;
+        p->nbx = p->nby = p->S;
+        p->team_threads = p->teams_per_cta = 0;
+        p->smem_bytes = 0;
+        return GRID_OK;
+    }
+    if (!lookup_kernel(p->cu, p->cv, p->P))
+        return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols", p->cu, p->cv, p->P);
+    // bin >= S + C - 1, multiple of the block
+    p->bin_u = round_up(p->S + p->cu - 1, p->cu);
+    p->bin_v = round_up(p->S + p->cv - 1, p->cv);
+    p->row_u = p->bin_u + p->cu - 1;
+    p->row_v = p->bin_v + p->cv - 1;
+    p->nbx = p->bin_u / p->cu;
+    p->nby = p->bin_v / p->cv;
+    p->team_threads = p->nbx * p->nby;
+    if (p->threads % 32 != 0 || p->threads < 32 || p->threads > 512)
+        return fail(GRID_ERR_UNSUPPORTED, "threads_per_cta %d must be a multiple of 32 in [32, 512]", p->threads);
+    if (p->team_threads > p->threads)
+        return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA has %d (tiles across CTAs are not built yet)",
+                    p->team_threads, p->threads);
+    if (p->batch < 1 || (p->batch & (p->batch - 1)) != 0)
+        return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two", p->batch);
+    if (p->chunk < 1) return fail(GRID_ERR_UNSUPPORTED, "chunk %d must be positive", p->chunk);
+    p->teams_per_cta = p->threads / p->team_threads;
+    size_t taps = (size_t)p->W * p->O * p->row_u * sizeof(float2);
+    if (p->cu != p->cv) taps += (size_t)p->W * p->O * p->row_v * sizeof(float2);
+    taps = (taps + 15) & ~(size_t)15;
+    const size_t per_team = (size_t)p->batch * (sizeof(SampleRec) + (size_t)p->P * sizeof(float2));
+    if (taps + per_team > (size_t)p->max_smem)
+        return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one batch buffer (%zu B) exceed %d B of shared memory",
+                    taps, per_team, p->max_smem);
+    // tiny bins: more teams than the batch buffers allow would not fit; idle the surplus threads
+    const size_t fit = ((size_t)p->max_smem - taps) / per_team;
+    if ((size_t)p->teams_per_cta > fit) p->teams_per_cta = (int)fit;
+    const size_t stage = (size_t)p->teams_per_cta * per_team;
+    p->smem_bytes = (int)(taps + stage);
+    return GRID_OK;
+}
+
+void default_tuning(grid_plan* p) {
+    p->variant = 1;
+    p->threads = 256;
+    p->batch = 64;
+    p->chunk = 1024;
+    p->ctas_per_sm = 2;
+    // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
+    if (p->P >= 4) {
+        if (p->S >= 24) { p->cu = 4; p->cv = 2; }
+        else if (p->S >= 12) { p->cu = 2; p->cv = 2; }
+        else { p->cu = 2; p->cv = 1; }
+    } else if (p->P == 2) {
+        if (p->S >= 24) { p->cu = 4; p->cv = 4; }
+        else { p->cu = 2; p->cv = 2; }
+    } else {
+        if (p->S >= 24) { p->cu = 8; p->cv = 4; }
+        else if (p->S >= 12) { p->cu = 4; p->cv = 4; }
+        else if (p->S >= 6) { p->cu = 4; p->cv = 2; }
+        else { p->cu = 2; p->cv = 2; }
+    }
+    if (p->S < 4) { p->cu = 1; p->cv = 1; }
+    // a bin must fit one CTA
+    while (derive(p) != GRID_OK && p->threads < 512) p->threads *= 2;
+}
+
+QuantParams quant_params(const grid_plan* p) {
+    QuantParams q;
+    q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
+    q.oversample = p->O;
+    q.shift = p->O - (p->O * p->S + 1) / 2;
+    q.q_limit = (p->N - p->S + 1) * p->O;
+    q.n_wplanes = p->W;
+    const bool scatter = p->variant == 0;
+    q.cu = scatter ? 1 : p->cu;
+    q.cv = scatter ? 1 : p->cv;
+    q.bin_u = p->bin_u; q.bin_v = p->bin_v; q.row_u = p->row_u; q.row_v = p->row_v;
+    return q;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* grid_last_error(void) { return g_err; }
+
+grid_plan* grid_plan_create(int grid_size, int support, int oversample, int n_wplanes, int n_pol) {
+    g_err[0] = 0;
+    if (grid_size < 1 || grid_size > 32767 || support < 1 || support > grid_size || support > 128 ||
+        oversample < 1 || n_wplanes < 1 || (long long)n_wplanes * oversample > 65535 ||
+        !(n_pol == 1 || n_pol == 2 || n_pol == 4) ||
+        (long long)(grid_size - support + 1) * oversample > 0x7fffffffLL) {
+        fail(GRID_ERR_INVALID_ARG, "grid_plan_create: invalid argument (N=%d S=%d O=%d W=%d P=%d)",
+             grid_size, support, oversample, n_wplanes, n_pol);
+        return nullptr;
+    }
+    // Without a device the plan can still be created and inspected (host logic); every compute
+    // entry point then fails with GRID_ERR_CUDA -- there is no CPU fallback.
+    int dev = 0, n_sm = 148, max_smem = 227 * 1024;
+    if (cudaGetDevice(&dev) == cudaSuccess) {
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    } else {
+        (void)cudaGetLastError();
+    }
+    grid_plan* p = new (std::nothrow) grid_plan();
+    if (!p) { fail(GRID_ERR_INVALID_ARG, "out of host memory"); return nullptr; }
+    memset(p, 0, sizeof(*p));
+    p->N = grid_size; p->S = support; p->O = oversample; p->W = n_wplanes; p->P = n_pol;
+    p->n_vis = -1;
+    p->n_sm = n_sm;
+    p->max_smem = max_smem - 1024;      // leave room for static shared memory
+    default_tuning(p);
+    if (derive(p) != GRID_OK) { delete p; return nullptr; }
+    return p;
+}
+
+void grid_plan_destroy(grid_plan* plan) { delete plan; }
+
+int grid_plan_set_samples(grid_plan* plan, long long n_vis) {
+    if (!plan || n_vis < 0) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_samples: invalid argument");
+    plan->n_vis = n_vis;
+    return GRID_OK;
+}
+
+int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_channels) {
+    if (!plan || n_baselines < 0 || n_times < 0 || n_channels < 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_layout: invalid argument");
+    plan->n_baselines = n_baselines; plan->n_times = n_times; plan->n_channels = n_channels;
+    return GRID_OK;
+}
+
+size_t grid_plan_workspace_bytes(const grid_plan* plan) {
+    if (!plan || plan->n_vis < 0) return 0;
+    return 256 + records_bytes(plan);
+}
+
+int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
+    if (!plan || (!dev_ptr && bytes) || ((uintptr_t)dev_ptr & 255) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_workspace: null or misaligned pointer");
+    plan->workspace = dev_ptr;
+    plan->workspace_bytes = bytes;
+    return GRID_OK;
+}
+
+int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threads_per_cta, int batch,
+                         int chunk, int ctas_per_sm) {
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: null plan");
+    grid_plan trial = *plan;
+    if (variant >= 0) trial.variant = variant;
+    if (cu > 0) trial.cu = cu;
+    if (cv > 0) trial.cv = cv;
+    if (threads_per_cta > 0) trial.threads = threads_per_cta;
+    if (batch > 0) trial.batch = batch;
+    if (chunk > 0) trial.chunk = chunk;
+    if (ctas_per_sm > 0) trial.ctas_per_sm = ctas_per_sm;
+    if (trial.variant != 0 && trial.variant != 1)
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: unknown variant %d", trial.variant);
+    const int rc = derive(&trial);
+    if (rc != GRID_OK) return rc;
+    *plan = trial;
+    return GRID_OK;
+}
+
+int grid_plan_get_info(const grid_plan* plan, int* out) {
+    if (!plan || !out) return fail(GRID_ERR_INVALID_ARG, "grid_plan_get_info: null argument");
+    const int v[16] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
+                       plan->teams_per_cta, plan->threads, plan->batch, plan->chunk, plan->ctas_per_sm,
+                       plan->smem_bytes, plan->n_sm, 0, 0, 0};
+    memcpy(out, v, sizeof(v));
+    return GRID_OK;
+}
+
+int grid_plan_last_launches(const grid_plan* plan) { return plan ? plan->last_launches : 0; }
+
+int grid_plan_set_kernel_events(grid_plan* plan, void* ev_start, void* ev_stop) {
+    if (!plan || ((ev_start == nullptr) != (ev_stop == nullptr)))
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_kernel_events: pass two events or two NULLs");
+    plan->ev_start = (cudaEvent_t)ev_start;
+    plan->ev_stop = (cudaEvent_t)ev_stop;
+    return GRID_OK;
+}
+
+int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid_stream_t stream) {
+    if (!plan || n < 0 || (n > 0 && (!uvw || !out)))
+        return fail(GRID_ERR_INVALID_ARG, "grid_quantise: invalid argument");
+    if (n == 0) return GRID_OK;
+    const long long blocks = (n + 255) / 256;
+    quantise_debug_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(uvw, out, n, quant_params(plan));
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_quantise: %s", cudaGetErrorString(e));
+    return GRID_OK;
+}
+
+int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                 const float* conv_kernel, float* grid, grid_stream_t stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute: call grid_plan_set_samples first");
+    if (plan->n_vis == 0) return GRID_OK;                              // R23
+    if (!uvw || !vis || !weights || !conv_kernel || !grid)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute: null array argument");
+    if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute: array arguments must be 16-byte aligned");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_execute: workspace missing or smaller than grid_plan_workspace_bytes()");
+
+    unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
+    SampleRec* recs = reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + 256);
+
+    // a1: quantise pass (also resets the chunk queue)
+    {
+        const long long threads = (plan->n_vis + 3) / 4;
+        const long long blocks = (threads + 255) / 256;
+        quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, plan->n_vis, quant_params(plan), counters);
+        plan->last_launches++;
+    }
+
+    GridParams gp;
+    memset(&gp, 0, sizeof(gp));
+    gp.recs = recs;
+    gp.vis = reinterpret_cast<const float2*>(vis);
+    gp.weights = weights;
+    gp.kern = reinterpret_cast<const float2*>(conv_kernel);
+    gp.grid = grid;
+    gp.counters = counters;
+    gp.n_vis = plan->n_vis;
+    gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
+    gp.bin_u = plan->bin_u; gp.bin_v = plan->bin_v; gp.row_u = plan->row_u; gp.row_v = plan->row_v;
+    gp.nbx = plan->nbx; gp.nby = plan->nby;
+    gp.team_threads = plan->team_threads; gp.teams_per_cta = plan->teams_per_cta;
+    gp.batch = plan->batch; gp.chunk = plan->chunk;
+    gp.n_outer = 1;
+
+    if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
+    if (plan->variant == 0) {
+        const long long total = plan->n_vis * plan->S;
+        const long long blocks = (total + 255) / 256;
+        if (blocks > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_execute: too many samples for the scatter variant");
+        if (plan->P == 1) grid_scatter_kernel<1><<<(unsigned)blocks, 256, 0, stream>>>(gp);
+        else if (plan->P == 2) grid_scatter_kernel<2><<<(unsigned)blocks, 256, 0, stream>>>(gp);
+        else grid_scatter_kernel<4><<<(unsigned)blocks, 256, 0, stream>>>(gp);
+        plan->last_launches++;
+    } else {
+        int shift = 0;
+        while ((1 << shift) < plan->batch) ++shift;
+        gp.batch_shift = shift;
+        // adaptive chunk length for small inputs: keep every SM busy
+        long long want_groups = (long long)plan->n_sm * plan->ctas_per_sm * 4;
+        long long per_group = (long long)plan->teams_per_cta * plan->chunk;
+        if ((plan->n_vis + per_group - 1) / per_group < want_groups) {
+            long long chunk = plan->n_vis / (want_groups * plan->teams_per_cta);
+            chunk = (chunk + plan->batch - 1) / plan->batch * plan->batch;
+            if (chunk < plan->batch) chunk = plan->batch;
+            if (chunk < gp.chunk) gp.chunk = (int)chunk;
+            per_group = (long long)plan->teams_per_cta * gp.chunk;
+        }
+        gp.n_groups = (plan->n_vis + per_group - 1) / per_group;
+        kernel_fn fn = lookup_kernel(plan->cu, plan->cv, plan->P);
+        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan->smem_bytes);
+        if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        long long ctas = (long long)plan->n_sm * plan->ctas_per_sm;
+        if (ctas > gp.n_groups) ctas = gp.n_groups;
+        fn<<<(unsigned)ctas, plan->threads, plan->smem_bytes, stream>>>(gp);
+        plan->last_launches++;
+    }
+    if (plan->ev_stop) cudaEventRecord(plan->ev_stop, stream);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: launch failed: %s", cudaGetErrorString(e));
+    return GRID_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,44 @@
+// Shared declarations of the B200 gridder (product path; never includes anything from oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gridb200 {
+
+// Quantised sample record written by the a1 pass ("the integer grid
+// coordinates, the sub-grid coordinates for indexing the GCF, the w plane index"), already in the
+// form the hot loop consumes for the plan's coarsening block (Cu x Cv) and bin (Bu x Bv):
+//   x: X0 | Y0 << 16   origin of the block-aligned bounding box, X0 = floor(i0/Cu)*Cu
+//                      0xFFFFFFFF marks a skipped sample (footprint outside the grid / non-finite)
+//   y: (X0 mod Bu) | (Y0 mod Bv) << 16
+//   z: element offset into the zero-padded u tap table: row(wp,su)*Lu + (Cu-1) - (i0-X0)
+//   w: element offset into the zero-padded v tap table: row(wp,sv)*Lv + (Cv-1) - (j0-Y0)
+typedef uint4 SampleRec;
+static constexpr uint32_t kInvalidRec = 0xFFFFFFFFu;
+
+struct QuantParams {
+    double c_centre;      // O*floor(N/2) + 0.5
+    int oversample;       // O
+    int shift;            // O - ceil(O*S/2)
+    int q_limit;          // (N-S+1)*O : valid iff 0 <= q < q_limit
+    int n_wplanes;
+    int cu, cv, bin_u, bin_v, row_u, row_v;   // coarsening block, bin, padded row lengths Lu, Lv
+};
+
+struct GridParams {
+    const SampleRec* recs;
+    const float2* vis;        // [n_vis][P]
+    const float* weights;     // [n_vis]
+    const float2* kern;       // [W][O][S]
+    float* grid;              // [N][N][P] complex64
+    unsigned int* counters;   // [0]: next chunk group
+    long long n_vis;
+    long long n_groups;
+    int N, S, n_rows;         // n_rows = W*O
+    int bin_u, bin_v, row_u, row_v, nbx, nby;
+    int team_threads, teams_per_cta, batch, chunk, batch_shift;
+    // traversal inside a chunk: idx(o, i) = i * n_outer + o, inner index serpentine (R: pin P11)
+    int n_outer;
+};
+
+}  // namespace gridb200

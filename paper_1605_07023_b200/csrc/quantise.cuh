@@ -1,0 +1,89 @@
+// Step a1: coordinate quantisation (device pass).  DESIGN.md R4, R5, R7.
+// The paper does this offline and hands the kernel "the integer grid coordinates, the sub-grid
+// coordinates for indexing the GCF, the w plane index" (section 4).
+#pragma once
+#include "gridder_common.cuh"
+
+namespace gridb200 {
+
+struct QuantOut { int i0, j0, su, sv, wp; bool valid; };
+
+// One axis: nearest 1/O cell (half up) in IEEE binary64 -- the product x*O is exact in binary64 and
+// the single rounding of the add cannot cross an integer (R4) -- then integer arithmetic.
+__device__ __forceinline__ bool quantise_axis(float x, const QuantParams& qp, int* cell, int* sub) {
+    const double pos = floor(fma((double)x, (double)qp.oversample, qp.c_centre));
+    const double q = pos + (double)qp.shift;
+    if (!(q >= 0.0 && q < (double)qp.q_limit)) return false;     // NaN, Inf, outside the grid
+    const int qi = (int)q;
+    const int c = qi / qp.oversample;
+    *cell = c;
+    *sub = qi - c * qp.oversample;
+    return true;
+}
+
+__device__ __forceinline__ QuantOut quantise_sample(float u, float v, float w, const QuantParams& qp) {
+    QuantOut r;
+    r.i0 = r.j0 = r.su = r.sv = r.wp = -1;
+    bool ok = quantise_axis(u, qp, &r.i0, &r.su);
+    ok = quantise_axis(v, qp, &r.j0, &r.sv) && ok;
+    const float aw = fabsf(w);
+    ok = ok && (aw <= 3.402823466e38f);                          // finite w (false for NaN)
+    // floor(|w|) clamped to the last plane (R5); comparison in float is exact for these integers
+    const int wp = (aw >= (float)(qp.n_wplanes - 1)) ? (qp.n_wplanes - 1) : (int)aw;
+    r.wp = wp;
+    r.valid = ok;
+    if (!ok) r.i0 = r.j0 = r.su = r.sv = r.wp = -1;
+    return r;
+}
+
+__device__ __forceinline__ SampleRec make_record(const QuantOut& q, const QuantParams& qp) {
+    SampleRec rec;
+    if (!q.valid) {
+        rec.x = kInvalidRec; rec.y = 0; rec.z = 0; rec.w = 0;
+        return rec;
+    }
+    const int X0 = (q.i0 / qp.cu) * qp.cu, Y0 = (q.j0 / qp.cv) * qp.cv;
+    rec.x = (uint32_t)X0 | ((uint32_t)Y0 << 16);
+    rec.y = (uint32_t)(X0 % qp.bin_u) | ((uint32_t)(Y0 % qp.bin_v) << 16);
+    rec.z = (uint32_t)((q.wp * qp.oversample + q.su) * qp.row_u + (qp.cu - 1) - (q.i0 - X0));
+    rec.w = (uint32_t)((q.wp * qp.oversample + q.sv) * qp.row_v + (qp.cv - 1) - (q.j0 - Y0));
+    return rec;
+}
+
+// uvw is [n][3] float32.  Each thread handles 4 consecutive samples = three aligned float4 loads.
+__global__ void __launch_bounds__(256)
+quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, long long n,
+                QuantParams qp, unsigned int* __restrict__ counters) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g == 0) counters[0] = 0;              // chunk-group queue of the gridding kernel
+    const long long first = g * 4;
+    if (first >= n) return;
+    float c[12];
+    if (first + 4 <= n) {
+        const float4* p = reinterpret_cast<const float4*>(uvw + first * 3);
+        const float4 a = __ldg(p), b = __ldg(p + 1), d = __ldg(p + 2);
+        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z;
+        c[7] = b.w; c[8] = d.x; c[9] = d.y; c[10] = d.z; c[11] = d.w;
+    } else {
+        for (int k = 0; k < 12; ++k) c[k] = (first * 3 + k < n * 3) ? __ldg(uvw + first * 3 + k) : 0.f;
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (first + k < n) {
+            const QuantOut q = quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp);
+            recs[first + k] = make_record(q, qp);
+        }
+    }
+}
+
+// Unpacked form for inspection / parity tests (grid_quantise): out[n][6].
+__global__ void __launch_bounds__(256)
+quantise_debug_kernel(const float* __restrict__ uvw, int* __restrict__ out, long long n, QuantParams qp) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n) return;
+    const QuantOut q = quantise_sample(uvw[3 * g], uvw[3 * g + 1], uvw[3 * g + 2], qp);
+    int* o = out + 6 * g;
+    o[0] = q.i0; o[1] = q.j0; o[2] = q.su; o[3] = q.sv; o[4] = q.wp; o[5] = q.valid ? 1 : 0;
+}
+
+}  // namespace gridb200

@@ -1,0 +1,99 @@
+"""-m "not gpu": the C-ABI library loads, exports every symbol include/grid.h declares, and its host
+logic (argument validation, bin / team derivation, workspace sizing) behaves as documented.
+No compute entry point is called here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    import __graft_entry__ as entry
+    entry.build()
+    from paper_1605_07023_b200 import binding as b
+    return b
+
+
+def test_header_symbols_are_exported(binding):
+    header = open(os.path.join(ROOT, "include", "grid.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(grid_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS), declared ^ set(binding.EXPORTS)
+    lib = ctypes.CDLL(binding.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_no_torch_types_in_header():
+    header = open(os.path.join(ROOT, "include", "grid.h")).read()
+    assert "torch" not in header.lower().replace("pytorch", "") and "at::" not in header
+
+
+def test_plan_validation(binding):
+    for args in [(0, 8, 8, 1, 4), (2048, 0, 8, 1, 4), (2048, 8, 0, 1, 4), (2048, 8, 8, 0, 4), (2048, 8, 8, 1, 3),
+                 (4, 8, 8, 1, 1), (40000, 8, 8, 1, 1), (2048, 8, 8, 70000, 1)]:
+        with pytest.raises(binding.GridError):
+            binding.GridPlan(*args)
+        assert binding.grid_last_error() != ""
+
+
+@pytest.mark.parametrize("S,P", [(7, 1), (8, 4), (16, 1), (8, 1), (4, 1), (4, 4), (16, 4), (32, 1), (32, 4), (1, 1)])
+def test_default_plan_geometry(binding, S, P):
+    plan = binding.GridPlan(4096, S, 8, 16, P)
+    i = plan.info()
+    # bin >= S + C - 1, aligned to the block; a team covers the bin exactly
+    assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
+    assert S + i["cu"] - 1 <= i["bin_u"] < S + 2 * i["cu"] - 1
+    assert S + i["cv"] - 1 <= i["bin_v"] < S + 2 * i["cv"] - 1
+    assert i["team_threads"] == (i["bin_u"] // i["cu"]) * (i["bin_v"] // i["cv"])
+    assert 1 <= i["teams_per_cta"] <= i["threads_per_cta"] // i["team_threads"]
+    assert i["cu"] * i["cv"] * P <= 32
+    assert i["smem_bytes"] <= 227 * 1024
+    plan.destroy()
+
+
+def test_workspace_and_tuning(binding):
+    plan = binding.GridPlan(2048, 8, 8, 1, 4)
+    assert plan.workspace_bytes() == 0              # set_samples not called yet
+    plan.set_samples(1001)
+    assert plan.workspace_bytes() == 256 + 1004 * 16
+    plan.set_samples(0)
+    assert plan.workspace_bytes() == 256
+    plan.set_layout(10, 10, 10)
+    plan.set_tuning(cu=2, cv=2, threads_per_cta=128, batch=32, chunk=512, ctas_per_sm=3)
+    i = plan.info()
+    assert (i["cu"], i["cv"], i["bin_u"], i["bin_v"], i["team_threads"], i["teams_per_cta"]) == (2, 2, 10, 10, 25, 5)
+    assert (i["batch"], i["chunk"], i["ctas_per_sm"]) == (32, 512, 3)
+    for bad in [dict(cu=3), dict(threads_per_cta=100), dict(batch=48), dict(cu=4, cv=4),   # 4x4x4 accumulators
+                dict(threads_per_cta=32, cu=1, cv=1), dict(batch=1 << 14)]:
+        with pytest.raises(binding.GridError) as e:
+            plan.set_tuning(**bad)
+        assert e.value.code == binding.GRID_ERR_UNSUPPORTED
+    assert plan.info() == i                          # failed overrides leave the plan unchanged
+    with pytest.raises(binding.GridError):
+        plan.set_samples(-1)
+    plan.destroy()
+
+
+def test_compute_calls_reject_host_memory(binding):
+    import torch
+    plan = binding.GridPlan(64, 8, 8, 1, 1)
+    plan.set_samples(4)
+    with pytest.raises(TypeError):                   # CPU tensors: no CPU fallback
+        plan.execute(torch.zeros(4, 3), torch.zeros(4, 1, dtype=torch.complex64), torch.zeros(4),
+                     torch.zeros(1, 8, 8, dtype=torch.complex64), torch.zeros(64, 64, 1, dtype=torch.complex64))
+    plan.destroy()
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1605_07023_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle", text, flags=re.M), f
+                assert "gridder_oracle" not in text, f

@@ -1,0 +1,187 @@
+"""-m gpu: the CUDA path (through the C ABI binding) against the float64 oracle, element by element,
+on the same seeded inputs.  Integer work (step a1) must be bit-exact; FP32 grids must satisfy
+rel-L2 <= 1e-5 and max-abs <= 1e-4 * max|grid| (BASELINE.json:north_star; R20)."""
+import numpy as np
+import pytest
+
+from paper_1605_07023_b200 import synth
+from gpu_util import assert_parity, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _quantise_gpu(N, S, O, W, uvw):
+    import torch
+    from paper_1605_07023_b200 import binding
+    plan = binding.GridPlan(N, S, O, W, 1)
+    try:
+        out = plan.quantise(torch.from_numpy(np.ascontiguousarray(uvw)).cuda())
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+    finally:
+        plan.destroy()
+
+
+def _check_quantise(oracle_mod, N, S, O, W, uvw):
+    got = _quantise_gpu(N, S, O, W, uvw)
+    ref = oracle_mod.quantise(N, S, O, W, uvw)
+    for col, key in enumerate(("i0", "j0", "su", "sv", "wp", "valid")):
+        assert np.array_equal(got[:, col], ref[key].astype(np.int32)), key
+    return int(ref["valid"].sum())
+
+
+@pytest.mark.parametrize("N,S,O,W", [(512, 7, 8, 1), (2048, 8, 8, 1), (4096, 16, 8, 32), (64, 5, 3, 2),
+                                     (33, 4, 5, 1), (16, 1, 1, 1), (8192, 32, 8, 16)])
+def test_quantise_bit_exact_random_and_ties(oracle_mod, N, S, O, W):
+    rng = np.random.default_rng(N + S)
+    n = 200_003
+    uvw = np.empty((n, 3), np.float32)
+    uvw[:, :2] = rng.uniform(-0.55 * N, 0.55 * N, (n, 2))
+    # exact ties between oversampled points, cell boundaries, tiny and huge values, non-finite
+    ties = ((rng.integers(-N * O, N * O, n // 4) + 0.5) / O).astype(np.float32)
+    uvw[: n // 4, 0] = ties
+    uvw[n // 4: n // 2, 1] = np.round(uvw[n // 4: n // 2, 1])
+    uvw[:, 2] = rng.uniform(-1.5 * W, 1.5 * W, n)
+    uvw[::97, 2] = np.round(uvw[::97, 2])
+    special = np.array([np.nan, np.inf, -np.inf, 1e30, -1e30, 1e-40, -1e-40, 0.0, -0.0], np.float32)
+    for k, v in enumerate(special):
+        uvw[1000 + 3 * k, 0] = v
+        uvw[1001 + 3 * k, 1] = v
+        uvw[1002 + 3 * k, 2] = v
+    nv = _check_quantise(oracle_mod, N, S, O, W, uvw)
+    assert 0 < nv < n
+
+
+def test_quantise_bit_exact_cfg0(oracle_mod):
+    wl = synth.make_workload(synth.get_config("cfg0"))
+    c = wl.cfg
+    assert _check_quantise(oracle_mod, c.grid_size, c.support, c.oversample, c.n_wplanes, wl.uvw) == c.n_vis
+
+
+def test_cfg0_full_parity(oracle_mod):
+    wl = synth.make_workload(synth.get_config("cfg0"))
+    c = wl.cfg
+    ref = oracle_mod.grid(c.grid_size, c.support, c.oversample, c.n_wplanes, c.n_pol, wl.uvw, wl.vis,
+                          wl.weights, wl.kernel)
+    for layout in (None, (c.n_baselines, c.n_times, c.n_chan)):
+        got, info = run_gpu(c.grid_size, c.support, c.oversample, c.n_wplanes, c.n_pol, wl.uvw, wl.vis,
+                            wl.weights, wl.kernel, layout=layout)
+        rel, mx = assert_parity(got, ref, f"cfg0 layout={layout}")
+        print(f"cfg0 layout={layout}: rel={rel:.2e} max={mx:.2e} {info}")
+
+
+COMBOS = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 1, 1), (4, 2, 1), (4, 4, 1), (8, 2, 1), (8, 4, 1),
+          (1, 1, 2), (2, 1, 2), (2, 2, 2), (4, 2, 2), (4, 4, 2),
+          (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 1, 4), (4, 2, 4)]
+
+
+@pytest.mark.parametrize("cu,cv,P", COMBOS)
+@pytest.mark.parametrize("S", [7, 8])
+def test_every_coarsening_block(oracle_mod, cu, cv, P, S):
+    # several chunks per team, a ragged tail (n not a multiple of batch, chunk or 4), samples that
+    # fall off the grid, two planes
+    N, O, W, n = 96, 8, 2, 30_001
+    uvw, vis, wts, kernel = synth.random_problem(100 * cu + 10 * cv + P + S, n, N, S, O, W, P,
+                                                 spread=0.5, walk=1.2)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                        tuning=dict(cu=cu, cv=cv, threads_per_cta=128, batch=32, chunk=200))
+    assert (info["cu"], info["cv"]) == (cu, cv)
+    assert_parity(got, ref, f"C={cu}x{cv} P={P} S={S}")
+
+
+@pytest.mark.parametrize("S,P,cu,cv", [(1, 1, 1, 1), (2, 4, 2, 1), (3, 1, 2, 2), (4, 1, 4, 2), (5, 2, 2, 2),
+                                       (16, 1, 4, 4), (16, 4, 2, 2), (32, 1, 8, 4), (32, 4, 4, 2), (13, 1, 4, 4)])
+def test_supports(oracle_mod, S, P, cu, cv):
+    N, O, W, n = 160, 4, 3, 12_345
+    uvw, vis, wts, kernel = synth.random_problem(7 * S + P, n, N, S, O, W, P, spread=0.48, walk=2.0)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(cu=cu, cv=cv, threads_per_cta=512))
+    assert_parity(got, ref, f"S={S} P={P} {info}")
+
+
+def test_default_tuning_all_config_shapes(oracle_mod):
+    # the (S, P, planes) of every BASELINE config with the plan's own default tuning, shrunk arrays
+    for name in ["cfg0", "cfg1", "cfg2", "cfg3"] + [f"cfg4_S{s}_P{p}" for s in (4, 8, 16, 32) for p in (1, 4)]:
+        cfg = synth.shrink(synth.get_config(name), n_ant=10, n_times=24, n_chan=12, grid_size=512)
+        wl = synth.make_workload(cfg)
+        ref = oracle_mod.grid(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                              wl.uvw, wl.vis, wl.weights, wl.kernel)
+        got, info = run_gpu(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                            wl.uvw, wl.vis, wl.weights, wl.kernel,
+                            layout=(cfg.n_baselines, cfg.n_times, cfg.n_chan))
+        rel, mx = assert_parity(got, ref, name)
+        print(f"{name}: rel={rel:.2e} max={mx:.2e} C={info['cu']}x{info['cv']}")
+
+
+def test_scatter_variant(oracle_mod):
+    N, S, O, W, P, n = 128, 6, 4, 2, 4, 5001
+    uvw, vis, wts, kernel = synth.random_problem(42, n, N, S, O, W, P, spread=0.52)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, _ = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(variant=0))
+    assert_parity(got, ref, "scatter")
+
+
+def test_edge_cases(oracle_mod):
+    import torch
+    from paper_1605_07023_b200 import binding
+    N, S, O, W, P = 64, 8, 8, 1, 4
+    kernel = synth.random_problem(1, 1, N, S, O, W, P)[3]
+    # n_vis = 0: no-op, grid untouched (R23)
+    init = (np.arange(N * N * P, dtype=np.float32).reshape(N, N, P) * (1 + 1j)).astype(np.complex64)
+    got, info = run_gpu(N, S, O, W, P, np.zeros((0, 3), np.float32), np.zeros((0, P), np.complex64),
+                        np.zeros(0, np.float32), kernel, grid_init=init)
+    assert np.array_equal(got, init) and info["launches"] == 0
+    # all samples invalid: grid untouched
+    uvw = np.full((100, 3), np.nan, np.float32)
+    uvw[50:] = 1e6
+    got, _ = run_gpu(N, S, O, W, P, uvw, np.ones((100, P), np.complex64), np.ones(100, np.float32), kernel,
+                     grid_init=init)
+    assert np.array_equal(got, init)
+    # accumulation into a non-zero grid (R10) and Inf visibilities on skipped samples must not leak
+    uvw, vis, wts, _ = synth.random_problem(3, 999, N, S, O, W, P, spread=0.7)
+    bad = oracle_mod.quantise(N, S, O, W, uvw)["valid"] == 0
+    assert bad.any()
+    vis[bad] = np.inf
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel) + init.astype(np.complex128)
+    got, _ = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, grid_init=init)
+    assert_parity(got, ref, "accumulate")
+    # single sample; footprint touching the grid corner; S = N
+    for (n_, s_, u, v) in [(64, 8, -28.0, -28.0), (64, 8, 27.4, 27.4), (8, 8, -1.0, -1.0)]:
+        k = synth.random_problem(5, 1, n_, s_, 2, 1, 1)[3]
+        one = np.array([[u, v, 0.0]], np.float32)
+        ref = oracle_mod.grid(n_, s_, 2, 1, 1, one, np.ones((1, 1), np.complex64), np.ones(1, np.float32), k)
+        assert np.count_nonzero(ref) == s_ * s_
+        got, _ = run_gpu(n_, s_, 2, 1, 1, one, np.ones((1, 1), np.complex64), np.ones(1, np.float32), k)
+        assert_parity(got, ref, f"single {n_} {s_}")
+    # error behaviour: missing set_samples / workspace, CPU tensors
+    plan = binding.GridPlan(N, S, O, W, P)
+    t = torch.zeros((4, 3), device="cuda")
+    with pytest.raises(binding.GridError):
+        plan.execute(t, t, t, t, t)
+    plan.set_samples(4)
+    with pytest.raises(binding.GridError):
+        plan.execute(torch.zeros((4, 3), device="cuda"), torch.zeros((4, P), dtype=torch.complex64, device="cuda"),
+                     torch.zeros(4, device="cuda"), torch.zeros((W, O, S), dtype=torch.complex64, device="cuda"),
+                     torch.zeros((N, N, P), dtype=torch.complex64, device="cuda"))
+    with pytest.raises(TypeError):
+        plan.execute(torch.zeros((4, 3)), t, t, t, t)
+    plan.destroy()
+
+
+def test_repeat_execute_accumulates(oracle_mod):
+    import torch
+    from paper_1605_07023_b200 import binding
+    N, S, O, W, P, n = 128, 8, 8, 2, 1, 20_000
+    uvw, vis, wts, kernel = synth.random_problem(77, n, N, S, O, W, P, spread=0.4, walk=1.0)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(n)
+    plan.allocate_workspace()
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device="cuda")
+    args = [torch.from_numpy(a).cuda() for a in (uvw, vis, wts, kernel)]
+    for _ in range(3):
+        plan.execute(*args, grid)
+    torch.cuda.synchronize()
+    plan.destroy()
+    assert_parity(grid.cpu().numpy(), 3 * ref, "3x execute")

@@ -90,8 +90,16 @@ int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid
 int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threads_per_cta,
                          int batch, int chunk, int ctas_per_sm);
 
+/* Order in which a chunk's samples are walked when the layout hint is set (the result is the same
+ * sum in a different order, pin P11): mode -1 = choose per call from the mean hop between
+ * consecutive samples measured by the quantise pass (default), 0 = input order (channel innermost,
+ * odd time rows mirrored), 1 = time innermost over blocks of `time_block` time steps (power of two,
+ * <= batch; 0 keeps the current value).  PAPER.md:61, 107: the gain of register accumulation depends
+ * on "the coordinates and ordering of the data". */
+int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block);
+
 /* HOST out[16]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
- * chunk, ctas_per_sm, smem_bytes, n_sm, traversal (0 input order, 1 time-inner), 0, 0. */
+ * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, 0. */
 int grid_plan_get_info(const grid_plan* plan, int* out);
 
 /* Measurement hook: two caller-owned cudaEvent_t (passed as void*) that the following grid_execute

@@ -16,7 +16,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
     "grid_plan_set_workspace", "grid_execute", "grid_quantise", "grid_plan_set_tuning",
-    "grid_plan_get_info", "grid_plan_set_kernel_events", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
+    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -37,6 +37,7 @@ _lib.grid_execute.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
 _lib.grid_plan_set_tuning.argtypes = [_vp] + [_int] * 7
 _lib.grid_plan_get_info.argtypes = [_vp, _vp]
+_lib.grid_plan_set_traversal.argtypes = [_vp, _int, _int]
 _lib.grid_plan_set_kernel_events.argtypes = [_vp, _vp, _vp]
 _lib.grid_plan_last_launches.argtypes = [_vp]
 _lib.grid_plan_destroy.argtypes = [_vp]
@@ -76,7 +77,7 @@ def _stream(stream):
 
 
 INFO_FIELDS = ("variant", "cu", "cv", "bin_u", "bin_v", "team_threads", "teams_per_cta",
-               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal")
+               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block")
 
 
 class GridPlan:
@@ -122,6 +123,9 @@ class GridPlan:
     def set_tuning(self, variant=-1, cu=0, cv=0, threads_per_cta=0, batch=0, chunk=0, ctas_per_sm=0):
         _check(_lib.grid_plan_set_tuning(self._h, variant, cu, cv, threads_per_cta, batch, chunk, ctas_per_sm),
                "grid_plan_set_tuning")
+
+    def set_traversal(self, mode=-1, time_block=0):
+        _check(_lib.grid_plan_set_traversal(self._h, mode, time_block), "grid_plan_set_traversal")
 
     def info(self) -> dict:
         out = (ctypes.c_int * 16)()
@@ -177,7 +181,11 @@ def grid_visibilities(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis
         if layout:
             plan.set_layout(*layout)
         if tuning:
-            plan.set_tuning(**tuning)
+            tuning = dict(tuning)
+            if "traversal" in tuning or "time_block" in tuning:
+                plan.set_traversal(tuning.pop("traversal", -1), tuning.pop("time_block", 0))
+            if tuning:
+                plan.set_tuning(**tuning)
         plan.allocate_workspace(uvw.device)
         if grid is None:
             grid = torch.zeros((grid_size, grid_size, n_pol), dtype=torch.complex64, device=uvw.device)

@@ -127,7 +127,23 @@ grid_coarsened_kernel(const GridParams gp) {
 #pragma unroll
             for (int q = 0; q < P; ++q) acc[r][c][q] = make_float2(0.f, 0.f);
 
-    const int n_batches = (gp.chunk + gp.batch - 1) / gp.batch;
+    // Traversal order inside a chunk (the sum is order-independent, pin P11):
+    //   mode 0: input order (channel innermost), odd time rows mirrored when the layout is known;
+    //   mode 1: a chunk is Tc time steps x all channels of one baseline, walked time-innermost,
+    //           serpentine.  Picked per call from the mean hop measured by the quantise pass.
+    int mode = gp.force_mode;
+    if (mode < 0) {
+        mode = 0;
+        if (gp.n_chan > 0) {
+            const float hc = __ldg(gp.hop_stats), ht = __ldg(gp.hop_stats + 1);
+            const float cost0 = ((gp.n_chan - 1) * hc + ht) / gp.n_chan;     // mean hop per sample
+            const float cost1 = ((gp.tc - 1) * ht + hc) / gp.tc;
+            mode = cost1 < cost0 ? 1 : 0;
+        }
+    }
+    const long long n_groups = mode ? gp.n_groups_b : gp.n_groups_a;
+    const int n_batches = mode ? (gp.n_chan + (1 << gp.cb_shift) - 1) >> gp.cb_shift
+                               : (gp.chunk + gp.batch - 1) / gp.batch;
     const int stage_total = gp.teams_per_cta * gp.batch;
 
     for (;;) {
@@ -135,20 +151,43 @@ grid_coarsened_kernel(const GridParams gp) {
         if (tid == 0) s_group = atomicAdd(gp.counters, 1u);          // a9: chunk-group queue
         __syncthreads();
         const long long group = s_group;
-        if (group >= gp.n_groups) break;
-        const long long group_start = group * (long long)gp.teams_per_cta * gp.chunk;
+        if (group >= n_groups) break;
         uint32_t cur = kInvalidRec;                                  // block currently in registers
 
         for (int b = 0; b < n_batches; ++b) {
             __syncthreads();
             // a2 + a3: stage one batch per team, pre-weighting the visibilities
-            for (int k = tid; k < stage_total; k += blockDim.x) {
-                const int t = k >> gp.batch_shift, s = k & (gp.batch - 1);
-                const int in_chunk = b * gp.batch + s;
-                const long long g = group_start + (long long)t * gp.chunk + in_chunk;
+            for (int kk = tid; kk < stage_total; kk += blockDim.x) {
+                const int t = kk >> gp.batch_shift, s = kk & (gp.batch - 1);
+                const long long chunk_id = group * gp.teams_per_cta + t;
+                long long g = -1;
+                int k = kk;                                          // shared-memory slot = traversal position
+                if (mode == 0) {
+                    const int in_chunk = b * gp.batch + s;
+                    long long a = chunk_id * gp.chunk + in_chunk;
+                    if (in_chunk < gp.chunk && a < gp.n_vis) {
+                        if (gp.n_chan > 0) {                         // mirror odd time rows (serpentine)
+                            const long long row = a / gp.n_chan;
+                            const int col = (int)(a - row * gp.n_chan);
+                            if (row & 1) a = row * gp.n_chan + (gp.n_chan - 1 - col);
+                        }
+                        g = a;
+                    }
+                } else if (chunk_id < gp.n_chunks_b) {
+                    // thread s -> (time ti, channel ci): consecutive threads read consecutive channels
+                    const int ti = s >> gp.cb_shift, ci = s & ((1 << gp.cb_shift) - 1);
+                    const int col = (b << gp.cb_shift) + ci;
+                    const long long bl = chunk_id / gp.n_tblocks;
+                    const int tb = (int)(chunk_id - bl * gp.n_tblocks);
+                    const int tabs = tb * gp.tc + ti;
+                    const int tt = (col & 1) ? gp.tc - 1 - ti : ti;
+                    k = (t << gp.batch_shift) + ci * gp.tc + tt;
+                    if (col < gp.n_chan && tabs < gp.n_times)
+                        g = (bl * gp.n_times + tabs) * (long long)gp.n_chan + col;
+                }
                 SampleRec rec;
                 rec.x = kInvalidRec; rec.y = rec.z = rec.w = 0;
-                if (in_chunk < gp.chunk && g < gp.n_vis) rec = __ldg(gp.recs + g);
+                if (g >= 0) rec = __ldg(gp.recs + g);
                 srec[k] = rec;
                 if (rec.x != kInvalidRec) {
                     const float w = __ldg(gp.weights + g);

@@ -37,6 +37,7 @@ struct grid_plan {
     size_t workspace_bytes;
     // tuning
     int variant, cu, cv, threads, batch, chunk, ctas_per_sm;
+    int traversal, time_block;      // -1 auto / 0 channel-innermost / 1 time-innermost; Tc
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
     int n_sm, max_smem;
@@ -112,6 +113,8 @@ void default_tuning(grid_plan* p) {
     p->batch = 64;
     p->chunk = 1024;
     p->ctas_per_sm = 2;
+    p->traversal = -1;
+    p->time_block = 16;
     // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
     if (p->P >= 4) {
         if (p->S >= 24) { p->cu = 4; p->cv = 2; }
@@ -233,8 +236,16 @@ int grid_plan_get_info(const grid_plan* plan, int* out) {
     if (!plan || !out) return fail(GRID_ERR_INVALID_ARG, "grid_plan_get_info: null argument");
     const int v[16] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
                        plan->teams_per_cta, plan->threads, plan->batch, plan->chunk, plan->ctas_per_sm,
-                       plan->smem_bytes, plan->n_sm, 0, 0, 0};
+                       plan->smem_bytes, plan->n_sm, plan->traversal, plan->time_block, 0};
     memcpy(out, v, sizeof(v));
+    return GRID_OK;
+}
+
+int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block) {
+    if (!plan || mode < -1 || mode > 1 || time_block < 0 || (time_block & (time_block - 1)) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_traversal: mode in {-1,0,1}, time_block a power of two or 0");
+    plan->traversal = mode;
+    if (time_block > 0) plan->time_block = time_block;
     return GRID_OK;
 }
 
@@ -276,11 +287,20 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
     SampleRec* recs = reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + 256);
 
-    // a1: quantise pass (also resets the chunk queue)
+    // the layout hint is used only if it is consistent with the sample count
+    const bool have_layout = plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
+                             (long long)plan->n_baselines * plan->n_times * plan->n_channels == plan->n_vis;
+    const int n_chan = have_layout ? plan->n_channels : 0, n_times = have_layout ? plan->n_times : 0;
+    float* hop_stats = reinterpret_cast<float*>(counters + 2);
+
+    // reset the chunk queue and the hop statistics, then a1: quantise pass
+    if (cudaMemsetAsync(counters, 0, 256, stream) != cudaSuccess)
+        return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
     {
         const long long threads = (plan->n_vis + 3) / 4;
         const long long blocks = (threads + 255) / 256;
-        quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, plan->n_vis, quant_params(plan), counters);
+        quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, plan->n_vis, quant_params(plan), hop_stats,
+                                                             n_chan, n_times, (float)(plan->bin_u + plan->bin_v));
         plan->last_launches++;
     }
 
@@ -298,7 +318,6 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     gp.nbx = plan->nbx; gp.nby = plan->nby;
     gp.team_threads = plan->team_threads; gp.teams_per_cta = plan->teams_per_cta;
     gp.batch = plan->batch; gp.chunk = plan->chunk;
-    gp.n_outer = 1;
 
     if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
     if (plan->variant == 0) {
@@ -323,12 +342,30 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
             if (chunk < gp.chunk) gp.chunk = (int)chunk;
             per_group = (long long)plan->teams_per_cta * gp.chunk;
         }
-        gp.n_groups = (plan->n_vis + per_group - 1) / per_group;
+        gp.n_groups_a = (plan->n_vis + per_group - 1) / per_group;
+        // time-innermost decomposition: chunk = tc time steps x all channels of one baseline
+        gp.hop_stats = hop_stats;
+        gp.force_mode = have_layout ? plan->traversal : 0;
+        gp.n_chan = n_chan; gp.n_times = n_times;
+        int tc = plan->time_block < plan->batch ? plan->time_block : plan->batch;
+        if (have_layout) {
+            while (tc > 1 && tc / 2 >= n_times) tc /= 2;
+            int tshift = 0;
+            while ((1 << tshift) < tc) ++tshift;
+            gp.tc = tc;
+            gp.cb_shift = shift - tshift;
+            gp.n_tblocks = (n_times + tc - 1) / tc;
+            gp.n_chunks_b = (long long)plan->n_baselines * gp.n_tblocks;
+            gp.n_groups_b = (gp.n_chunks_b + plan->teams_per_cta - 1) / plan->teams_per_cta;
+        } else {
+            gp.tc = 1; gp.n_tblocks = 1;
+        }
+        const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         kernel_fn fn = lookup_kernel(plan->cu, plan->cv, plan->P);
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan->smem_bytes);
         if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         long long ctas = (long long)plan->n_sm * plan->ctas_per_sm;
-        if (ctas > gp.n_groups) ctas = gp.n_groups;
+        if (ctas > max_groups) ctas = max_groups;
         fn<<<(unsigned)ctas, plan->threads, plan->smem_bytes, stream>>>(gp);
         plan->last_launches++;
     }

@@ -32,13 +32,16 @@ struct GridParams {
     const float2* kern;       // [W][O][S]
     float* grid;              // [N][N][P] complex64
     unsigned int* counters;   // [0]: next chunk group
+    const float* hop_stats;   // [0] mean-hop sum along channels, [1] along time (quantise pass)
     long long n_vis;
-    long long n_groups;
+    long long n_groups_a, n_groups_b, n_chunks_b;   // mode 0 / mode 1 work decomposition
     int N, S, n_rows;         // n_rows = W*O
     int bin_u, bin_v, row_u, row_v, nbx, nby;
     int team_threads, teams_per_cta, batch, chunk, batch_shift;
-    // traversal inside a chunk: idx(o, i) = i * n_outer + o, inner index serpentine (R: pin P11)
-    int n_outer;
+    // layout hint (0 = unknown) and time-innermost traversal: a mode-1 chunk is tc time steps x all
+    // channels of one baseline; a batch is tc x (1 << cb_shift) samples
+    int n_chan, n_times, tc, cb_shift, n_tblocks;
+    int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
 };
 
 }  // namespace gridb200

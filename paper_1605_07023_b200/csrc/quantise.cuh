@@ -51,12 +51,37 @@ __device__ __forceinline__ SampleRec make_record(const QuantOut& q, const QuantP
 }
 
 // uvw is [n][3] float32.  Each thread handles 4 consecutive samples = three aligned float4 loads.
+// It also measures, on every 64th block, how far consecutive samples move along the channel axis and
+// along the time axis (layout hint: sample = (baseline*n_times + t)*n_chan + c), so that the gridding
+// kernel can walk each chunk along the slower axis (hop_stats[0] channel, [1] time; capped per hop).
 __global__ void __launch_bounds__(256)
 quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, long long n,
-                QuantParams qp, unsigned int* __restrict__ counters) {
+                QuantParams qp, float* __restrict__ hop_stats, int n_chan, int n_times, float hop_cap) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g == 0) counters[0] = 0;              // chunk-group queue of the gridding kernel
     const long long first = g * 4;
+    if (n_chan > 0 && (blockIdx.x & 63) == 0) {
+        float hc = 0.f, ht = 0.f;
+        if (first < n) {
+            const long long row = first / n_chan;
+            const int col = (int)(first - row * n_chan);
+            const int t = (int)(row % n_times);
+            const float u = __ldg(uvw + 3 * first), v = __ldg(uvw + 3 * first + 1);
+            if (col + 1 < n_chan)
+                hc = fminf(fabsf(__ldg(uvw + 3 * (first + 1)) - u) + fabsf(__ldg(uvw + 3 * (first + 1) + 1) - v), hop_cap);
+            if (t + 1 < n_times)
+                ht = fminf(fabsf(__ldg(uvw + 3 * (first + n_chan)) - u) + fabsf(__ldg(uvw + 3 * (first + n_chan) + 1) - v), hop_cap);
+            if (!(hc == hc)) hc = 0.f;           // NaN coordinates carry no information
+            if (!(ht == ht)) ht = 0.f;
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            hc += __shfl_xor_sync(0xffffffffu, hc, o);
+            ht += __shfl_xor_sync(0xffffffffu, ht, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(hop_stats, hc);
+            atomicAdd(hop_stats + 1, ht);
+        }
+    }
     if (first >= n) return;
     float c[12];
     if (first + 4 <= n) {

@@ -17,7 +17,11 @@ def run_gpu(N, S, O, W, P, uvw, vis, weights, kernel, layout=None, tuning=None, 
         if layout:
             plan.set_layout(*layout)
         if tuning:
-            plan.set_tuning(**tuning)
+            tuning = dict(tuning)
+            if "traversal" in tuning or "time_block" in tuning:
+                plan.set_traversal(tuning.pop("traversal", -1), tuning.pop("time_block", 0))
+            if tuning:
+                plan.set_tuning(**tuning)
         plan.allocate_workspace(dev)
         if grid_init is None:
             grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)

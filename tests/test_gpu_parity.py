@@ -114,6 +114,34 @@ def test_default_tuning_all_config_shapes(oracle_mod):
         print(f"{name}: rel={rel:.2e} max={mx:.2e} C={info['cu']}x{info['cv']}")
 
 
+@pytest.mark.parametrize("mode", [-1, 0, 1])
+@pytest.mark.parametrize("n_ant,n_times,n_chan,tc", [(9, 37, 13, 16), (7, 5, 64, 16), (12, 64, 3, 8), (6, 33, 40, 32)])
+def test_traversal_modes(oracle_mod, mode, n_ant, n_times, n_chan, tc):
+    # ragged time blocks (n_times % tc != 0), channel counts that are not a multiple of the batch
+    # columns, fewer time steps than one block
+    for name in ("cfg1", "cfg2"):
+        cfg = synth.shrink(synth.get_config(name), n_ant=n_ant, n_times=n_times, n_chan=n_chan, grid_size=384)
+        wl = synth.make_workload(cfg)
+        ref = oracle_mod.grid(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                              wl.uvw, wl.vis, wl.weights, wl.kernel)
+        got, info = run_gpu(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                            wl.uvw, wl.vis, wl.weights, wl.kernel,
+                            layout=(cfg.n_baselines, cfg.n_times, cfg.n_chan),
+                            tuning=dict(traversal=mode, time_block=tc, threads_per_cta=128))
+        assert (info["traversal"], info["time_block"]) == (mode, tc)
+        assert_parity(got, ref, f"{name} mode={mode}")
+
+
+def test_inconsistent_layout_hint_is_ignored(oracle_mod):
+    cfg = synth.shrink(synth.get_config("cfg1"), n_ant=8, n_times=16, n_chan=8, grid_size=256)
+    wl = synth.make_workload(cfg)
+    ref = oracle_mod.grid(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                          wl.uvw, wl.vis, wl.weights, wl.kernel)
+    got, _ = run_gpu(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                     wl.uvw, wl.vis, wl.weights, wl.kernel, layout=(3, 5, 7), tuning=dict(traversal=1))
+    assert_parity(got, ref, "bad layout")
+
+
 def test_scatter_variant(oracle_mod):
     N, S, O, W, P, n = 128, 6, 4, 2, 4, 5001
     uvw, vis, wts, kernel = synth.random_problem(42, n, N, S, O, W, P, spread=0.52)
@@ -164,8 +192,10 @@ def test_edge_cases(oracle_mod):
         plan.execute(torch.zeros((4, 3), device="cuda"), torch.zeros((4, P), dtype=torch.complex64, device="cuda"),
                      torch.zeros(4, device="cuda"), torch.zeros((W, O, S), dtype=torch.complex64, device="cuda"),
                      torch.zeros((N, N, P), dtype=torch.complex64, device="cuda"))
-    with pytest.raises(TypeError):
-        plan.execute(torch.zeros((4, 3)), t, t, t, t)
+    with pytest.raises(TypeError):                    # host memory is rejected: no CPU fallback
+        plan.execute(torch.zeros((4, 3)), torch.zeros((4, P), dtype=torch.complex64, device="cuda"),
+                     torch.zeros(4, device="cuda"), torch.zeros((W, O, S), dtype=torch.complex64, device="cuda"),
+                     torch.zeros((N, N, P), dtype=torch.complex64, device="cuda"))
     plan.destroy()
 
 

@@ -7,6 +7,7 @@
 #include <cstring>
 #include <new>
 
+#include "grid_cyclic_kernel.cuh"
 #include "grid_kernel.cuh"
 #include "gridder_common.cuh"
 #include "quantise.cuh"
@@ -62,6 +63,37 @@ kernel_fn lookup_kernel(int cu, int cv, int P) {
     return nullptr;
 }
 
+template <int CU, int CV, int P, int LOGS, bool OK = (CU <= (1 << LOGS) && CV <= (1 << LOGS))>
+struct CycPick { static kernel_fn get() { return grid_cyclic_kernel<CU, CV, P, LOGS>; } };
+template <int CU, int CV, int P, int LOGS>
+struct CycPick<CU, CV, P, LOGS, false> { static kernel_fn get() { return nullptr; } };
+
+template <int CU, int CV, int P>
+kernel_fn pick_cyc(int logs) {
+    switch (logs) {
+        case 2: return CycPick<CU, CV, P, 2>::get();
+        case 3: return CycPick<CU, CV, P, 3>::get();
+        case 4: return CycPick<CU, CV, P, 4>::get();
+        case 5: return CycPick<CU, CV, P, 5>::get();
+    }
+    return nullptr;
+}
+
+// Power-of-two supports 4..32 (bin == support, no padding).
+kernel_fn lookup_cyclic(int cu, int cv, int P, int logs) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_cyc<a, b, p>(logs);
+    CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
+    CASE(1, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2)
+    CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+    return nullptr;
+}
+
+int log2_exact(int v) {
+    for (int l = 0; l < 31; ++l) if ((1 << l) == v) return l;
+    return -1;
+}
+
 size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec); }
 
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
@@ -71,6 +103,38 @@ int derive(grid_plan* p) {
         p->nbx = p->nby = p->S;
         p->team_threads = p->teams_per_cta = 0;
         p->smem_bytes = 0;
+        return GRID_OK;
+    }
+    if (p->variant == 2) {
+        const int logs = log2_exact(p->S);
+        if (logs < 2 || logs > 5)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 2 needs a power-of-two support in [4, 32], got %d", p->S);
+        if (!lookup_cyclic(p->cu, p->cv, p->P, logs))
+            return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols, support %d",
+                        p->cu, p->cv, p->P, p->S);
+        if ((long long)p->W * p->O * 3 * p->S + 2 * p->S > 65535)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 2: tap table too large for 16-bit offsets");
+        p->bin_u = p->bin_v = p->S;
+        p->row_u = p->row_v = 3 * p->S;
+        p->nbx = p->S / p->cu;
+        p->nby = p->S / p->cv;
+        p->team_threads = p->nbx * p->nby;
+        if (p->threads % 32 != 0 || p->threads < 32 || p->threads > 512)
+            return fail(GRID_ERR_UNSUPPORTED, "threads_per_cta %d must be a multiple of 32 in [32, 512]", p->threads);
+        if (p->team_threads > p->threads)
+            return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA has %d", p->team_threads, p->threads);
+        if (p->batch < 1 || (p->batch & (p->batch - 1)) != 0)
+            return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two", p->batch);
+        if (p->chunk < 1) return fail(GRID_ERR_UNSUPPORTED, "chunk %d must be positive", p->chunk);
+        p->teams_per_cta = p->threads / p->team_threads;
+        size_t taps = ((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15;
+        const size_t per_team = (size_t)p->batch * (sizeof(uint4) + (size_t)p->P * sizeof(float2));
+        if (taps + per_team > (size_t)p->max_smem)
+            return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one batch buffer (%zu B) exceed %d B of shared memory",
+                        taps, per_team, p->max_smem);
+        const size_t fit = ((size_t)p->max_smem - taps) / per_team;
+        if ((size_t)p->teams_per_cta > fit) p->teams_per_cta = (int)fit;
+        p->smem_bytes = (int)(taps + (size_t)p->teams_per_cta * per_team);
         return GRID_OK;
     }
     if (!lookup_kernel(p->cu, p->cv, p->P))
@@ -130,12 +194,23 @@ void default_tuning(grid_plan* p) {
         else { p->cu = 2; p->cv = 2; }
     }
     if (p->S < 4) { p->cu = 1; p->cv = 1; }
+    // power-of-two supports: bin == support, no padding (grid_cyclic_kernel.cuh)
+    const int logs = log2_exact(p->S);
+    if (logs >= 2 && logs <= 5) {
+        grid_plan trial = *p;
+        trial.variant = 2;
+        if (trial.P >= 4) { trial.cu = 2; trial.cv = 2; }
+        else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = 2; }
+        else { trial.cu = 4; trial.cv = (logs >= 3) ? 4 : 2; }
+        if (derive(&trial) == GRID_OK) { *p = trial; return; }
+    }
     // a bin must fit one CTA
     while (derive(p) != GRID_OK && p->threads < 512) p->threads *= 2;
 }
 
 QuantParams quant_params(const grid_plan* p) {
     QuantParams q;
+    q.format = p->variant == 2 ? 1 : 0;
     q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
     q.oversample = p->O;
     q.shift = p->O - (p->O * p->S + 1) / 2;
@@ -224,7 +299,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     if (batch > 0) trial.batch = batch;
     if (chunk > 0) trial.chunk = chunk;
     if (ctas_per_sm > 0) trial.ctas_per_sm = ctas_per_sm;
-    if (trial.variant != 0 && trial.variant != 1)
+    if (trial.variant < 0 || trial.variant > 2)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: unknown variant %d", trial.variant);
     const int rc = derive(&trial);
     if (rc != GRID_OK) return rc;
@@ -361,7 +436,8 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
             gp.tc = 1; gp.n_tblocks = 1;
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
-        kernel_fn fn = lookup_kernel(plan->cu, plan->cv, plan->P);
+        kernel_fn fn = plan->variant == 2 ? lookup_cyclic(plan->cu, plan->cv, plan->P, log2_exact(plan->S))
+                                          : lookup_kernel(plan->cu, plan->cv, plan->P);
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan->smem_bytes);
         if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         long long ctas = (long long)plan->n_sm * plan->ctas_per_sm;

@@ -13,12 +13,13 @@ struct QuantOut { int i0, j0, su, sv, wp; bool valid; };
 __device__ __forceinline__ bool quantise_axis(float x, const QuantParams& qp, int* cell, int* sub) {
     const double pos = floor(fma((double)x, (double)qp.oversample, qp.c_centre));
     const double q = pos + (double)qp.shift;
-    if (!(q >= 0.0 && q < (double)qp.q_limit)) return false;     // NaN, Inf, outside the grid
-    const int qi = (int)q;
+    const bool ok = (q >= 0.0 && q < (double)qp.q_limit);        // false for NaN, Inf, outside the grid
+    // skipped samples still get in-grid coordinates (fmax/fmin drop NaN): the cyclic kernel walks them
+    const int qi = (int)fmin(fmax(q, 0.0), (double)(qp.q_limit - 1));
     const int c = qi / qp.oversample;
     *cell = c;
     *sub = qi - c * qp.oversample;
-    return true;
+    return ok;
 }
 
 __device__ __forceinline__ QuantOut quantise_sample(float u, float v, float w, const QuantParams& qp) {
@@ -32,8 +33,14 @@ __device__ __forceinline__ QuantOut quantise_sample(float u, float v, float w, c
     const int wp = (aw >= (float)(qp.n_wplanes - 1)) ? (qp.n_wplanes - 1) : (int)aw;
     r.wp = wp;
     r.valid = ok;
-    if (!ok) r.i0 = r.j0 = r.su = r.sv = r.wp = -1;
     return r;
+}
+
+__device__ __forceinline__ CycRec make_cyc_record(const QuantOut& q, const QuantParams& qp) {
+    CycRec rec;
+    rec.pos = (uint32_t)q.i0 | ((uint32_t)q.j0 << 16) | (q.valid ? 0u : 0x8000u);
+    rec.rows = (uint32_t)(q.wp * qp.oversample + q.su) | ((uint32_t)(q.wp * qp.oversample + q.sv) << 16);
+    return rec;
 }
 
 __device__ __forceinline__ SampleRec make_record(const QuantOut& q, const QuantParams& qp) {
@@ -96,7 +103,8 @@ quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, lon
     for (int k = 0; k < 4; ++k) {
         if (first + k < n) {
             const QuantOut q = quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp);
-            recs[first + k] = make_record(q, qp);
+            if (qp.format == 0) recs[first + k] = make_record(q, qp);
+            else reinterpret_cast<CycRec*>(recs)[first + k] = make_cyc_record(q, qp);
         }
     }
 }
@@ -108,7 +116,9 @@ quantise_debug_kernel(const float* __restrict__ uvw, int* __restrict__ out, long
     if (g >= n) return;
     const QuantOut q = quantise_sample(uvw[3 * g], uvw[3 * g + 1], uvw[3 * g + 2], qp);
     int* o = out + 6 * g;
-    o[0] = q.i0; o[1] = q.j0; o[2] = q.su; o[3] = q.sv; o[4] = q.wp; o[5] = q.valid ? 1 : 0;
+    const int m = q.valid ? 0 : -1;               // skipped samples report -1 (their clamped walk
+    o[0] = q.i0 | m; o[1] = q.j0 | m; o[2] = q.su | m; o[3] = q.sv | m; o[4] = q.wp | m;   // coordinates are internal)
+    o[5] = q.valid ? 1 : 0;
 }
 
 }  // namespace gridb200

@@ -45,10 +45,14 @@ def test_plan_validation(binding):
 def test_default_plan_geometry(binding, S, P):
     plan = binding.GridPlan(4096, S, 8, 16, P)
     i = plan.info()
-    # bin >= S + C - 1, aligned to the block; a team covers the bin exactly
-    assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
-    assert S + i["cu"] - 1 <= i["bin_u"] < S + 2 * i["cu"] - 1
-    assert S + i["cv"] - 1 <= i["bin_v"] < S + 2 * i["cv"] - 1
+    if i["variant"] == 2:
+        # power-of-two support: bin == support, owned positions S/C apart (north_star: "taken modulo the support")
+        assert S in (4, 8, 16, 32) and i["bin_u"] == i["bin_v"] == S
+    else:
+        # bin >= S + C - 1, aligned to the block; a team covers the bin exactly
+        assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
+        assert S + i["cu"] - 1 <= i["bin_u"] < S + 2 * i["cu"] - 1
+        assert S + i["cv"] - 1 <= i["bin_v"] < S + 2 * i["cv"] - 1
     assert i["team_threads"] == (i["bin_u"] // i["cu"]) * (i["bin_v"] // i["cv"])
     assert 1 <= i["teams_per_cta"] <= i["threads_per_cta"] // i["team_threads"]
     assert i["cu"] * i["cv"] * P <= 32
@@ -64,7 +68,7 @@ def test_workspace_and_tuning(binding):
     plan.set_samples(0)
     assert plan.workspace_bytes() == 256
     plan.set_layout(10, 10, 10)
-    plan.set_tuning(cu=2, cv=2, threads_per_cta=128, batch=32, chunk=512, ctas_per_sm=3)
+    plan.set_tuning(variant=1, cu=2, cv=2, threads_per_cta=128, batch=32, chunk=512, ctas_per_sm=3)
     i = plan.info()
     assert (i["cu"], i["cv"], i["bin_u"], i["bin_v"], i["team_threads"], i["teams_per_cta"]) == (2, 2, 10, 10, 25, 5)
     assert (i["batch"], i["chunk"], i["ctas_per_sm"]) == (32, 512, 3)

@@ -85,9 +85,33 @@ def test_every_coarsening_block(oracle_mod, cu, cv, P, S):
                                                  spread=0.5, walk=1.2)
     ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
     got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
-                        tuning=dict(cu=cu, cv=cv, threads_per_cta=128, batch=32, chunk=200))
-    assert (info["cu"], info["cv"]) == (cu, cv)
+                        tuning=dict(variant=1, cu=cu, cv=cv, threads_per_cta=128, batch=32, chunk=200))
+    assert (info["variant"], info["cu"], info["cv"]) == (1, cu, cv)
     assert_parity(got, ref, f"C={cu}x{cv} P={P} S={S}")
+
+
+CYCLIC = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (1, 1, 2), (2, 2, 2), (4, 2, 2),
+          (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 2, 4)]
+
+
+@pytest.mark.parametrize("cu,cv,P", CYCLIC)
+@pytest.mark.parametrize("S", [4, 8, 16, 32])
+def test_every_cyclic_block(oracle_mod, cu, cv, P, S):
+    # bin == support kernel (variant 2): ragged tail, samples off the grid (walked with zero
+    # visibilities), jumps larger than the support, three planes
+    if cu > S or cv > S:
+        pytest.skip("block larger than the support")
+    N, O, W, n = 128, 4, 3, 20_003
+    uvw, vis, wts, kernel = synth.random_problem(1000 + 100 * cu + 10 * cv + P + S, n, N, S, O, W, P,
+                                                 spread=0.5, walk=1.5)
+    uvw[5000:5100, :2] = np.random.default_rng(S).uniform(-60, 60, (100, 2))    # big jumps
+    uvw[7000:7010, 0] = np.nan
+    vis[7000:7010] = np.inf
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                        tuning=dict(variant=2, cu=cu, cv=cv, threads_per_cta=128, batch=32, chunk=300))
+    assert (info["variant"], info["cu"], info["cv"], info["bin_u"]) == (2, cu, cv, S)
+    assert_parity(got, ref, f"cyclic C={cu}x{cv} P={P} S={S}")
 
 
 @pytest.mark.parametrize("S,P,cu,cv", [(1, 1, 1, 1), (2, 4, 2, 1), (3, 1, 2, 2), (4, 1, 4, 2), (5, 2, 2, 2),
@@ -96,7 +120,8 @@ def test_supports(oracle_mod, S, P, cu, cv):
     N, O, W, n = 160, 4, 3, 12_345
     uvw, vis, wts, kernel = synth.random_problem(7 * S + P, n, N, S, O, W, P, spread=0.48, walk=2.0)
     ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
-    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(cu=cu, cv=cv, threads_per_cta=512))
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                        tuning=dict(variant=1, cu=cu, cv=cv, threads_per_cta=512))
     assert_parity(got, ref, f"S={S} P={P} {info}")
 
 

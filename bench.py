@@ -163,6 +163,24 @@ def parse_tuning(text):
     return out
 
 
+def rank_config(cfg, rank):
+    """Shard of rank `rank`: the same recipe with its own seed (an independent problem per GPU)."""
+    from dataclasses import replace
+    return cfg if rank == 0 else replace(cfg, seed=cfg.seed + 1000 * rank)
+
+
+def reduce_over_ranks(times_ms, units, device, world):
+    """MAX of the device times and SUM of the units processed over all ranks (the only exchange)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), device=device, dtype=torch.float64)
+    tot = torch.tensor([float(units)], device=device, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.tolist()], float(tot.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -180,10 +198,7 @@ def run_ours(args):
 
     # Weak scaling: every rank grids its own full workload (same recipe, seed + rank) onto its own
     # grid -- independent problems like the paper's W-stacking slices; no collective.
-    cfg = synth.get_config(args.config)
-    if rank > 0:
-        from dataclasses import replace
-        cfg = replace(cfg, seed=cfg.seed + 1000 * rank)
+    cfg = rank_config(synth.get_config(args.config), rank)
     wl = synth.make_workload(cfg)
     N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
 
@@ -265,13 +280,8 @@ def run_ours(args):
         e2e_ms = e0.elapsed_time(e1)
         e2e = {"ms": e2e_ms, "steps": e_steps, "h2d": h2d, "d2h": d2h}
 
-    t = torch.tensor([elapsed_ms, e2e["ms"] / e2e["steps"] if e2e else 0.0, kernel_ms], device=dev, dtype=torch.float64)
-    tot = torch.tensor([float(updates_per_step)], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    elapsed_ms, e2e_step_ms, kernel_ms = (float(x) for x in t.tolist())
-    total_updates_per_step = float(tot.item())
+    (elapsed_ms, e2e_step_ms, kernel_ms), total_updates_per_step = reduce_over_ranks(
+        [elapsed_ms, e2e["ms"] / e2e["steps"] if e2e else 0.0, kernel_ms], updates_per_step, dev, world)
 
     if rank == 0:
         value = total_updates_per_step * args.steps / (elapsed_ms * 1e-3)

@@ -71,6 +71,40 @@ __device__ __forceinline__ uint32_t moved_mask(int from, int to) {
     return m & ALL;
 }
 
+// One grid point (all polarisations): if `hit`, atomically add the accumulators and zero them.
+template <int P>
+__device__ __forceinline__ void flush_cell(float2 (&a)[P], float* p, uint32_t hit) {
+    if constexpr (P == 4) {
+        asm volatile(
+            "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %9, 0;\n\t"
+            "@q red.relaxed.gpu.global.add.v4.f32 [%8], {%0, %1, %2, %3};\n\t"
+            "@q red.relaxed.gpu.global.add.v4.f32 [%8+16], {%4, %5, %6, %7};\n\t"
+            "@q mov.f32 %0, 0f00000000;\n\t@q mov.f32 %1, 0f00000000;\n\t"
+            "@q mov.f32 %2, 0f00000000;\n\t@q mov.f32 %3, 0f00000000;\n\t"
+            "@q mov.f32 %4, 0f00000000;\n\t@q mov.f32 %5, 0f00000000;\n\t"
+            "@q mov.f32 %6, 0f00000000;\n\t@q mov.f32 %7, 0f00000000;\n\t}"
+            : "+f"(a[0].x), "+f"(a[0].y), "+f"(a[1].x), "+f"(a[1].y), "+f"(a[2].x), "+f"(a[2].y),
+              "+f"(a[3].x), "+f"(a[3].y)
+            : "l"(p), "r"(hit) : "memory");
+    } else if constexpr (P == 2) {
+        asm volatile(
+            "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %5, 0;\n\t"
+            "@q red.relaxed.gpu.global.add.v4.f32 [%4], {%0, %1, %2, %3};\n\t"
+            "@q mov.f32 %0, 0f00000000;\n\t@q mov.f32 %1, 0f00000000;\n\t"
+            "@q mov.f32 %2, 0f00000000;\n\t@q mov.f32 %3, 0f00000000;\n\t}"
+            : "+f"(a[0].x), "+f"(a[0].y), "+f"(a[1].x), "+f"(a[1].y)
+            : "l"(p), "r"(hit) : "memory");
+    } else {
+        static_assert(P == 1, "1, 2 or 4 polarisations");
+        asm volatile(
+            "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+            "@q red.relaxed.gpu.global.add.v2.f32 [%2], {%0, %1};\n\t"
+            "@q mov.f32 %0, 0f00000000;\n\t@q mov.f32 %1, 0f00000000;\n\t}"
+            : "+f"(a[0].x), "+f"(a[0].y)
+            : "l"(p), "r"(hit) : "memory");
+    }
+}
+
 template <int CU, int CV, int P, int LOGS>
 __global__ void __launch_bounds__(512, 1)
 grid_cyclic_kernel(const GridParams gp) {
@@ -129,19 +163,11 @@ grid_cyclic_kernel(const GridParams gp) {
         for (int b = 0; b < CV; ++b) {
 #pragma unroll
             for (int a = 0; a < CU; ++a) {
-                if (((mx >> (r0 + a * DU)) | (my >> (s0 + b * DV))) & 1u) {
-                    float* p = gp.grid + ((size_t)yb[b] * gp.N + xa[a]) * (2 * P);
-                    if constexpr (P % 2 == 0) {
-#pragma unroll
-                        for (int q = 0; q < P; q += 2)
-                            red_add_v4(p + 2 * q, acc[b][a][q].x, acc[b][a][q].y, acc[b][a][q + 1].x, acc[b][a][q + 1].y);
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < P; ++q) red_add_v2(p + 2 * q, acc[b][a][q].x, acc[b][a][q].y);
-                    }
-#pragma unroll
-                    for (int q = 0; q < P; ++q) acc[b][a][q] = make_float2(0.f, 0.f);
-                }
+                // predicated, in place (no branch, no temporaries: cf. the register-pressure note PAPER.md:93-95)
+                const uint32_t hit = ((mx >> (r0 + a * DU)) | (my >> (s0 + b * DV))) & 1u;
+                const uint32_t cellidx = (uint32_t)(yb[b] * gp.N + xa[a]);          // < 2^30
+                float* p = gp.grid + (size_t)cellidx * (2 * P);
+                flush_cell<P>(acc[b][a], p, hit);
             }
         }
     };

@@ -1,0 +1,76 @@
+"""-m gpu: BASELINE.json's configs at FULL size, in the launch configuration bench.py times (plan
+defaults + layout hint), against the float64 oracle on what it can compute in seconds:
+  * sampled outputs: bands of grid rows (centre, mid-radius, outer) computed exactly by the oracle
+    (its row-restricted mode scans every sample), compared element by element with the north_star
+    tolerances, the max-abs one relative to the band's own maximum (stricter than max|grid|);
+  * a property that holds at any size (pin P3): with V = 1 the sum of the grid equals
+    sum_n weight_n * ksum[wp][sv] * ksum[wp][su]; a lost or doubled chunk of 1024 samples moves it by
+    3e-5, the bound is 1e-5 of the sum of the terms' moduli;
+  * step a1 bit-exact on a strided sample of the full uvw array.
+"""
+import numpy as np
+import pytest
+
+from paper_1605_07023_b200 import synth
+from gpu_util import REL_L2_TOL, MAX_ABS_TOL
+
+pytestmark = pytest.mark.gpu
+
+FULL = ["cfg1", "cfg2", "cfg3", "cfg4_S4_P1", "cfg4_S32_P4", "cfg4_S16_P1"]
+
+
+def _bands(N, S):
+    c = N // 2
+    return [(c - 8, c + 8), (c + N // 8, c + N // 8 + 8), (c - int(0.4 * N), c - int(0.4 * N) + 8)]
+
+
+@pytest.mark.parametrize("name", FULL)
+def test_full_size(oracle_mod, name):
+    import torch
+    from paper_1605_07023_b200 import binding
+    cfg = synth.get_config(name)
+    wl = synth.make_workload(cfg)
+    N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
+    dev = torch.device("cuda:0")
+    d_uvw, d_vis, d_w, d_k = (torch.from_numpy(a).to(dev) for a in (wl.uvw, wl.vis, wl.weights, wl.kernel))
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(cfg.n_vis)
+    plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    plan.allocate_workspace(dev)
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+    plan.execute(d_uvw, d_vis, d_w, d_k, grid)
+    torch.cuda.synchronize()
+
+    # a1 on a strided sample of the full array: bit-exact
+    step = 997
+    q_gpu = plan.quantise(d_uvw[::step].contiguous()).cpu().numpy()
+    q_ref = oracle_mod.quantise(N, S, O, W, wl.uvw[::step])
+    for col, key in enumerate(("i0", "j0", "su", "sv", "wp", "valid")):
+        assert np.array_equal(q_gpu[:, col], q_ref[key].astype(np.int32)), key
+
+    # sampled outputs: exact row bands
+    for lo, hi in _bands(N, S):
+        ref = oracle_mod.grid(N, S, O, W, P, wl.uvw, wl.vis, wl.weights, wl.kernel, rows=(lo, hi))
+        got = grid[lo:hi].cpu().numpy().astype(np.complex128)
+        nref = np.linalg.norm(ref.ravel())
+        assert nref > 0, f"{name}: empty band {lo}:{hi}"
+        rel = np.linalg.norm((got - ref).ravel()) / nref
+        mx = np.abs(got - ref).max() / np.abs(ref).max()
+        print(f"{name} rows {lo}:{hi} rel_l2={rel:.2e} max_abs/max={mx:.2e}")
+        assert rel <= REL_L2_TOL and mx <= MAX_ABS_TOL, (name, lo, hi, rel, mx)
+
+    # property at full size: V = 1  =>  sum(grid) = sum_n w_n * ksum_v * ksum_u
+    ones = torch.ones_like(d_vis)
+    grid.zero_()
+    plan.execute(d_uvw, ones, d_w, d_k, grid)
+    torch.cuda.synchronize()
+    total = grid.to(torch.complex128).sum(dim=(0, 1)).cpu().numpy()
+    q = oracle_mod.quantise(N, S, O, W, wl.uvw)
+    ok = q["valid"] == 1
+    ksum = wl.kernel.astype(np.complex128).sum(axis=2)                 # [W][O]
+    terms = wl.weights[ok].astype(np.float64) * ksum[q["wp"][ok], q["sv"][ok]] * ksum[q["wp"][ok], q["su"][ok]]
+    expect, scale = terms.sum(), np.abs(terms).sum()
+    err = np.abs(total - expect).max() / scale
+    print(f"{name} sum property: err/scale={err:.2e} n_valid={int(ok.sum())}")
+    assert err <= 1e-5, (name, err)
+    plan.destroy()

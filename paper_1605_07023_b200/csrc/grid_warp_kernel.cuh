@@ -1,0 +1,430 @@
+// Steps a2-a9, power-of-two supports: the warp-autonomous gridding kernel (variant 3).
+//
+// Work distribution is Romein's: a thread is responsible for all grid points with a
+// fixed position modulo the bin and keeps the one inside the current footprint in a register
+// accumulator, flushing it with an atomic add when it changes.  Thread coarsening:
+// each thread owns Cu x Cv positions, so tap loads, the "did my points move" test and the loop
+// overhead are paid once per block of Cu*Cv*P accumulators.  As in grid_cyclic_kernel.cuh the bin
+// equals the support (no zero padding) and the Cu (Cv) positions of a thread are S/Cu (S/Cv) apart.
+//
+// What is new relative to the paper's kernel and to variant 2, and why (B200 measurements in
+// DESIGN.md section 6):
+//   * on sm_100a integer/logic instructions cost 1.5-2 issue cycles against 1 for an FFMA, so the
+//     flush path decides the rate once samples hop by a cell or more (BASELINE.json's data: 0.6
+//     columns + 0.5 rows per sample).  The flush is therefore organised by moved COLUMN and moved ROW
+//     of the bin: a one-cell move makes the owning threads execute Cv (or Cu) cell bodies, not
+//     Cu*Cv, and the grid coordinates of the owned points are kept in registers and updated only
+//     for the points that moved (no per-flush recomputation);
+//   * a team never spans more than it must: a *group* is max(1, team/32) warps; groups share
+//     nothing but the tap table, take chunks from the queue on their own and
+//     synchronise only among their own warps -- no CTA-wide barrier in steady state;
+//   * batches are staged by cp.async (LDGSTS) into a two-stage raw ring, then "cooked" in shared
+//     memory by the group's own lanes (pre-weighting PAPER.md:91, tap offsets, moved masks) while the
+//     next batch is in flight.
+#pragma once
+#include "gridder_common.cuh"
+#include "grid_cyclic_kernel.cuh"      // moved_mask<>, flush helpers
+
+namespace gridb200 {
+
+struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
+    long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)
+    int len;                  // mode 0: positions in the chunk
+    int h;                    // mode 1: time steps in this block (0: empty chunk)
+    int col0, rowpar;         // mode 0 with layout: column of `base` and parity of its time row
+    int pad0, pad1;
+};
+
+__device__ __forceinline__ void cp_async_4(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_8(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int CU, int CV, int P, int LOGS>
+struct WarpKernelTraits {
+    static constexpr int S = 1 << LOGS;
+    static constexpr int DU = S / CU, DV = S / CV;       // spacing of a thread's owned positions
+    static constexpr int TEAM = DU * DV;                  // threads per bin
+    static constexpr int GW = TEAM > 32 ? TEAM / 32 : 1;  // warps per group
+    static constexpr int GT = GW * 32;                    // threads per group
+    static constexpr int TPG = TEAM >= 32 ? 1 : 32 / TEAM;    // teams (chunks in flight) per group
+    static constexpr int ACC = 2 * CU * CV * P;
+    static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
+    // shared memory of one group for a batch of B samples per team
+    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + 8 * P); }
+    __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
+    __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
+    __host__ __device__ static constexpr size_t group_bytes(int B) {
+        return (cooked_bytes(B) + 2 * raw_bytes(B) + ctrl_bytes() + 15) & ~(size_t)15;
+    }
+};
+
+template <int CU, int CV, int P, int LOGS>
+__global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS>::MAX_THREADS), 1)
+grid_warp_kernel(const GridParams gp) {
+    using T = WarpKernelTraits<CU, CV, P, LOGS>;
+    constexpr int S = T::S, DU = T::DU, DV = T::DV, TEAM = T::TEAM, GW = T::GW, GT = T::GT, TPG = T::TPG;
+    constexpr int ROW = 3 * S;                         // tripled tap row: k[t mod S], t < 3S
+    constexpr bool WIDE = S > 16;                      // record format: 32-bit masks need two words
+    static_assert(CU <= S && CV <= S, "block larger than the support");
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* taps = reinterpret_cast<float2*>(smem_raw);
+    const size_t taps_bytes = ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
+    const int B = gp.batch, bshift = gp.batch_shift;
+    const int slots = TPG * B;
+
+    const int tid = threadIdx.x;
+    const int group = tid / GT, lg = tid - group * GT;
+    unsigned char* gbase = smem_raw + taps_bytes + (size_t)group * T::group_bytes(B);
+    uint4* crec = reinterpret_cast<uint4*>(gbase);                                       // cooked records
+    float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)slots * 16);                // cooked vis
+    unsigned char* rbase = gbase + T::cooked_bytes(B);
+    const size_t rstage = T::raw_bytes(B);
+    // raw stage layout: vis [slots][P] float2, rec [slots] 8 B, weights [slots] float
+    WarpChunk* geom = reinterpret_cast<WarpChunk*>(rbase + 2 * rstage);                  // [2][TPG]
+    uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
+    uint32_t* ctrl = last_pos + 2 * TPG;
+
+    for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {          // a4
+        const int r = k / ROW, t = (k - r * ROW) & (S - 1);
+        taps[k] = __ldg(gp.kern + (size_t)r * S + t);
+    }
+    __syncthreads();
+    if (group >= gp.groups_per_cta) return;            // surplus threads (CTA not a multiple of GT)
+
+    auto group_sync = [&]() {
+        if constexpr (GW == 1) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" :: "r"(group + 1), "r"(GT) : "memory");
+    };
+
+    // a5: ownership
+    const int tg = (TPG > 1) ? lg / TEAM : 0;          // my team within the group
+    const int lt = lg - tg * TEAM;
+    const int r0 = lt % DU, s0 = lt / DU;
+    uint32_t MX = 0, MY = 0;
+#pragma unroll
+    for (int a = 0; a < CU; ++a) MX |= 1u << (r0 + a * DU);
+#pragma unroll
+    for (int b = 0; b < CV; ++b) MY |= 1u << (s0 + b * DV);
+    const uint32_t MXY = MX | (MY << 16);              // !WIDE: both masks in one word
+    const uint4* my_rec = crec + (size_t)tg * B;
+    const float2* my_vis = cvis + (size_t)tg * B * P;
+    const unsigned char* my_tu = reinterpret_cast<const unsigned char*>(taps + r0);
+    const unsigned char* my_tv = reinterpret_cast<const unsigned char*>(taps + s0);
+    const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
+
+    float2 acc[CV][CU][P];
+#pragma unroll
+    for (int b = 0; b < CV; ++b)
+#pragma unroll
+        for (int a = 0; a < CU; ++a)
+#pragma unroll
+            for (int q = 0; q < P; ++q) acc[b][a][q] = make_float2(0.f, 0.f);
+    int cx[CU];                     // x of the grid point currently held for owned column a
+    uint32_t ry[CV];                // y * N of the grid point currently held for owned row b
+#pragma unroll
+    for (int a = 0; a < CU; ++a) cx[a] = 0;
+#pragma unroll
+    for (int b = 0; b < CV; ++b) ry[b] = 0;
+
+    // a8: one grid point, all polarisations: atomic add, then clear
+    auto flush_point = [&](float2 (&v)[P], uint32_t cell) {
+        float* p = gp.grid + (size_t)cell * (2 * P);
+        if constexpr (P == 4) {
+            red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
+            red_add_v4(p + 4, v[2].x, v[2].y, v[3].x, v[3].y);
+        } else if constexpr (P == 2) {
+            red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
+        } else {
+            red_add_v2(p, v[0].x, v[0].y);
+        }
+#pragma unroll
+        for (int q = 0; q < P; ++q) v[q] = make_float2(0.f, 0.f);
+    };
+
+    int mode = gp.force_mode;
+    if (mode < 0) {
+        mode = 0;
+        if (gp.n_chan > 0) {
+            const float hc = __ldg(gp.hop_stats), ht = __ldg(gp.hop_stats + 1);
+            const float cost0 = ((gp.n_chan - 1) * hc + ht) / gp.n_chan;
+            const float cost1 = ((gp.tc - 1) * ht + hc) / gp.tc;
+            mode = cost1 < cost0 ? 1 : 0;
+        }
+    }
+    const long long n_groups = mode ? gp.n_groups_b : gp.n_groups_a;
+    const int n_batches = mode ? (gp.n_chan + (1 << gp.cb_shift) - 1) >> gp.cb_shift
+                               : (gp.chunk + B - 1) >> bshift;
+
+    // a9: take the next chunk group from the queue; lanes t < TPG work out their team's geometry
+    auto fetch = [&](int par) -> long long {
+        uint32_t v = 0;
+        if constexpr (GW == 1) {
+            if (lg == 0) v = atomicAdd(gp.counters, 1u);
+            v = __shfl_sync(0xffffffffu, v, 0);
+        } else {
+            if (lg == 0) ctrl[0] = atomicAdd(gp.counters, 1u);
+            group_sync();
+            v = ctrl[0];
+        }
+        const long long g = v;
+        if (g < n_groups && lg < TPG) {
+            const long long chunk_id = g * TPG + lg;
+            WarpChunk cg;
+            cg.base = 0; cg.len = 0; cg.h = 0; cg.col0 = 0; cg.rowpar = 0; cg.pad0 = cg.pad1 = 0;
+            if (mode == 0) {
+                cg.base = chunk_id * gp.chunk;
+                const long long left = gp.n_vis - cg.base;
+                cg.len = left <= 0 ? 0 : (left < gp.chunk ? (int)left : gp.chunk);
+                if (gp.n_chan > 0) {
+                    const long long row = cg.base / gp.n_chan;
+                    cg.col0 = (int)(cg.base - row * gp.n_chan);
+                    cg.rowpar = (int)(row & 1);
+                }
+            } else if (chunk_id < gp.n_chunks_b) {
+                const long long bl = chunk_id / gp.n_tblocks;
+                const int tb = (int)(chunk_id - bl * gp.n_tblocks);
+                cg.h = gp.n_times - tb * gp.tc < gp.tc ? gp.n_times - tb * gp.tc : gp.tc;
+                cg.base = (bl * gp.n_times + (long long)tb * gp.tc) * gp.n_chan;
+            }
+            geom[par * TPG + lg] = cg;
+        }
+        group_sync();
+        return g;
+    };
+
+    auto count_of = [&](const WarpChunk& cg, int b) -> int {
+        if (mode == 0) {
+            const int left = cg.len - (b << bshift);
+            return left < 0 ? 0 : (left < B ? left : B);
+        }
+        int cols = gp.n_chan - (b << gp.cb_shift);
+        if (cols > (1 << gp.cb_shift)) cols = 1 << gp.cb_shift;
+        return cols < 0 ? 0 : cols * cg.h;
+    };
+
+    auto sample_of = [&](const WarpChunk& cg, int b, int k) -> long long {
+        if (mode == 0) {
+            const int off = (b << bshift) + k;
+            long long a = cg.base + off;
+            if (gp.n_chan > 0) {                        // serpentine over time rows
+                const uint32_t col = (uint32_t)(cg.col0 + off);
+                const uint32_t radd = col / (uint32_t)gp.n_chan;
+                const int colr = (int)(col - radd * (uint32_t)gp.n_chan);
+                if ((cg.rowpar + radd) & 1u) a += gp.n_chan - 1 - 2 * colr;
+            }
+            return a;
+        }
+        const int ci = (int)((uint32_t)k / (uint32_t)cg.h), tt = k - ci * cg.h;
+        const int col = (b << gp.cb_shift) + ci;
+        const int ti = (col & 1) ? cg.h - 1 - tt : tt;
+        return cg.base + (long long)ti * gp.n_chan + col;
+    };
+
+    // a3: start the copies of batch b of the chunk group `par` into raw stage `st`
+    auto issue = [&](int par, int b, int st) {
+        unsigned char* rs = rbase + (size_t)st * rstage;
+        float2* rvis = reinterpret_cast<float2*>(rs);
+        CycRec* rrec = reinterpret_cast<CycRec*>(rs + (size_t)slots * 8 * P);
+        float* rw = reinterpret_cast<float*>(rs + (size_t)slots * (8 * P + 8));
+        for (int kk = lg; kk < slots; kk += GT) {
+            const int t = kk >> bshift, k = kk & (B - 1);
+            const WarpChunk cg = geom[par * TPG + t];
+            if (k >= count_of(cg, b)) continue;
+            const long long g = sample_of(cg, b, k);
+            cp_async_8(rrec + kk, recs + g);
+            cp_async_4(rw + kk, gp.weights + g);
+            if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
+            else {
+#pragma unroll
+                for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + g * P + q);
+            }
+        }
+        cp_async_commit();
+    };
+
+    // a2: raw stage -> cooked records (tap offsets, moved masks) and pre-weighted visibilities
+    auto cook = [&](int par, int b, int st) {
+        const unsigned char* rs = rbase + (size_t)st * rstage;
+        const float2* rvis = reinterpret_cast<const float2*>(rs);
+        const CycRec* rrec = reinterpret_cast<const CycRec*>(rs + (size_t)slots * 8 * P);
+        const float* rw = reinterpret_cast<const float*>(rs + (size_t)slots * (8 * P + 8));
+        for (int kk = lg; kk < slots; kk += GT) {
+            const int t = kk >> bshift, k = kk & (B - 1);
+            const WarpChunk cg = geom[par * TPG + t];
+            const int cnt = count_of(cg, b);
+            uint4 c = make_uint4(0u, 0u, 0u, 0u);
+            float w = 0.f;
+            bool valid = false;
+            if (k < cnt) {
+                const CycRec rec = rrec[kk];
+                uint32_t mx = 0, my = 0;
+                if (k > 0 || b > 0) {
+                    const uint32_t pp = k > 0 ? rrec[kk - 1].pos : last_pos[((b - 1) & 1) * TPG + t];
+                    mx = moved_mask<LOGS>((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
+                    my = moved_mask<LOGS>((int)(pp >> 16), (int)(rec.pos >> 16));
+                }
+                if (k == cnt - 1) last_pos[(b & 1) * TPG + t] = rec.pos;
+                const int i0 = (int)(rec.pos & 0x7fffu), j0 = (int)(rec.pos >> 16);
+                const uint32_t xo = (rec.rows & 0xffffu) * ROW + S - (i0 & (S - 1));
+                const uint32_t yo = (rec.rows >> 16) * ROW + S - (j0 & (S - 1));
+                c.x = rec.pos & 0xffff7fffu;
+                if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
+                else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
+                valid = (rec.pos & 0x8000u) == 0;
+                if (valid) w = rw[kk];
+            }
+            crec[kk] = c;
+#pragma unroll
+            for (int q = 0; q < P; ++q) {
+                float2 v = make_float2(0.f, 0.f);
+                if (valid) { v = rvis[(size_t)kk * P + q]; v.x *= w; v.y *= w; }
+                cvis[(size_t)kk * P + q] = v;
+            }
+        }
+    };
+
+    int par = 0;
+    long long cur = fetch(par);
+    if (cur < n_groups) issue(par, 0, 0);
+    int st = 0;                                        // raw stage holding the next batch to cook
+    while (cur < n_groups) {
+        const WarpChunk my_cg = geom[par * TPG + tg];
+        bool live = false;
+        long long next = cur;
+        int next_par = par;
+        for (int b = 0; b < n_batches; ++b) {
+            cp_async_wait_all();
+            group_sync();                              // raw batch visible; previous hot loop done
+            cook(par, b, st);
+            group_sync();                              // cooked batch visible; raw stage consumed
+            if (b + 1 < n_batches) {
+                issue(par, b + 1, st ^ 1);
+            } else {                                   // prefetch the first batch of the next group
+                next_par = par ^ 1;
+                next = fetch(next_par);
+                if (next < n_groups) issue(next_par, 0, st ^ 1);
+            }
+            st ^= 1;
+
+            int cnt = count_of(my_cg, b);
+            if (b == 0 && cnt > 0) {                   // first sample of the chunk: take position
+                live = true;
+                const uint32_t p0 = my_rec[0].x;
+                const int i0 = (int)(p0 & 0x7fffu), j0 = (int)(p0 >> 16);
+#pragma unroll
+                for (int a = 0; a < CU; ++a) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+#pragma unroll
+                for (int bb = 0; bb < CV; ++bb) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+            }
+            if constexpr (TPG > 1) cnt = __reduce_max_sync(0xffffffffu, cnt);
+
+            for (int s = 0; s < cnt; ++s) {
+                const uint4 c = my_rec[s];
+                bool moved;
+                if constexpr (WIDE) moved = ((c.z & MX) | (c.w & MY)) != 0;
+                else moved = (c.w & MXY) != 0;
+                if (moved) {                           // a5/a8: some of my points moved
+                    const int i0 = (int)(c.x & 0x7fffu), j0 = (int)(c.x >> 16);
+                    const uint32_t mxs = (WIDE ? c.z : c.w) >> r0;
+                    const uint32_t mys = (WIDE ? c.w : (c.w >> 16)) >> s0;
+#pragma unroll
+                    for (int a = 0; a < CU; ++a) {
+                        if (mxs & (1u << (a * DU))) {  // owned column a left the footprint
+#pragma unroll
+                            for (int bb = 0; bb < CV; ++bb) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                            cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+                        }
+                    }
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb) {
+                        if (mys & (1u << (bb * DV))) { // owned row bb left the footprint
+#pragma unroll
+                            for (int a = 0; a < CU; ++a)
+                                if (!(mxs & (1u << (a * DU)))) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                            ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                        }
+                    }
+                }
+                const float2* tu;
+                const float2* tv;
+                if constexpr (WIDE) {
+                    tu = reinterpret_cast<const float2*>(my_tu) + (c.y & 0xffffu);
+                    tv = reinterpret_cast<const float2*>(my_tv) + (c.y >> 16);
+                } else {
+                    tu = reinterpret_cast<const float2*>(my_tu + c.y);
+                    tv = reinterpret_cast<const float2*>(my_tv + c.z);
+                }
+                float2 gu[CU], gv[CV], v[P];
+#pragma unroll
+                for (int a = 0; a < CU; ++a) gu[a] = tu[a * DU];
+#pragma unroll
+                for (int bb = 0; bb < CV; ++bb) gv[bb] = tv[bb * DV];
+                if constexpr (P == 4) {
+                    const float4 v01 = *reinterpret_cast<const float4*>(my_vis + s * 4);
+                    const float4 v23 = *reinterpret_cast<const float4*>(my_vis + s * 4 + 2);
+                    v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
+                    v[2] = make_float2(v23.x, v23.y); v[3] = make_float2(v23.z, v23.w);
+                } else if constexpr (P == 2) {
+                    const float4 v01 = *reinterpret_cast<const float4*>(my_vis + s * 2);
+                    v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
+                } else {
+                    v[0] = my_vis[s];
+                }
+                if constexpr (P < CU) {
+                    // a6 reordered: T = Gv_j * V_p first, then Gu_i * T
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb) {
+#pragma unroll
+                        for (int q = 0; q < P; ++q) {
+                            const float tr = gv[bb].x * v[q].x - gv[bb].y * v[q].y;
+                            const float ti = gv[bb].x * v[q].y + gv[bb].y * v[q].x;
+#pragma unroll
+                            for (int a = 0; a < CU; ++a) {                               // a7
+                                acc[bb][a][q].x = fmaf(gu[a].x, tr, acc[bb][a][q].x);
+                                acc[bb][a][q].x = fmaf(-gu[a].y, ti, acc[bb][a][q].x);
+                                acc[bb][a][q].y = fmaf(gu[a].x, ti, acc[bb][a][q].y);
+                                acc[bb][a][q].y = fmaf(gu[a].y, tr, acc[bb][a][q].y);
+                            }
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb) {
+#pragma unroll
+                        for (int a = 0; a < CU; ++a) {
+                            const float gr = gv[bb].x * gu[a].x - gv[bb].y * gu[a].y;       // a6
+                            const float gi = gv[bb].x * gu[a].y + gv[bb].y * gu[a].x;
+#pragma unroll
+                            for (int q = 0; q < P; ++q) {                                    // a7
+                                acc[bb][a][q].x = fmaf(gr, v[q].x, acc[bb][a][q].x);
+                                acc[bb][a][q].x = fmaf(-gi, v[q].y, acc[bb][a][q].x);
+                                acc[bb][a][q].y = fmaf(gr, v[q].y, acc[bb][a][q].y);
+                                acc[bb][a][q].y = fmaf(gi, v[q].x, acc[bb][a][q].y);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        if (live) {                                    // end of chunk: everything goes to the grid
+#pragma unroll
+            for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                for (int a = 0; a < CU; ++a) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+        }
+        cur = next;
+        par = next_par;
+    }
+    cp_async_wait_all();
+}
+
+}  // namespace gridb200

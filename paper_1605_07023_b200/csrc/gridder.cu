@@ -9,6 +9,7 @@
 
 #include "grid_cyclic_kernel.cuh"
 #include "grid_kernel.cuh"
+#include "grid_warp_kernel.cuh"
 #include "gridder_common.cuh"
 #include "quantise.cuh"
 
@@ -41,6 +42,7 @@ struct grid_plan {
     int traversal, time_block;      // -1 auto / 0 channel-innermost / 1 time-innermost; Tc
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
+    int groups_per_cta, queue_teams;      // variant 3: warp groups per CTA; teams per queue entry (all variants)
     int n_sm, max_smem;
     int last_launches;
     cudaEvent_t ev_start, ev_stop;
@@ -89,6 +91,43 @@ kernel_fn lookup_cyclic(int cu, int cv, int P, int logs) {
     return nullptr;
 }
 
+// Variant 3 (grid_warp_kernel.cuh): kernel + the compile-time geometry the host needs.
+struct WarpDesc {
+    kernel_fn fn;
+    int gt, tpg, team, max_threads;
+    size_t (*group_bytes)(int);
+};
+
+template <int CU, int CV, int P, int LOGS, bool OK = (CU <= (1 << LOGS) && CV <= (1 << LOGS))>
+struct WarpPick {
+    static WarpDesc get() {
+        using T = WarpKernelTraits<CU, CV, P, LOGS>;
+        return WarpDesc{grid_warp_kernel<CU, CV, P, LOGS>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes};
+    }
+};
+template <int CU, int CV, int P, int LOGS>
+struct WarpPick<CU, CV, P, LOGS, false> { static WarpDesc get() { return WarpDesc{nullptr, 0, 0, 0, 0, nullptr}; } };
+
+template <int CU, int CV, int P>
+WarpDesc pick_warp(int logs) {
+    switch (logs) {
+        case 2: return WarpPick<CU, CV, P, 2>::get();
+        case 3: return WarpPick<CU, CV, P, 3>::get();
+        case 4: return WarpPick<CU, CV, P, 4>::get();
+        case 5: return WarpPick<CU, CV, P, 5>::get();
+    }
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+WarpDesc lookup_warp(int cu, int cv, int P, int logs) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_warp<a, b, p>(logs);
+    CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
+    CASE(1, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
+    CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
 int log2_exact(int v) {
     for (int l = 0; l < 31; ++l) if ((1 << l) == v) return l;
     return -1;
@@ -103,6 +142,47 @@ int derive(grid_plan* p) {
         p->nbx = p->nby = p->S;
         p->team_threads = p->teams_per_cta = 0;
         p->smem_bytes = 0;
+        return GRID_OK;
+    }
+    p->groups_per_cta = 0;
+    if (p->variant == 3) {
+        const int logs = log2_exact(p->S);
+        if (logs < 2 || logs > 5)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 32], got %d", p->S);
+        const WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs);
+        if (!d.fn)
+            return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols, support %d",
+                        p->cu, p->cv, p->P, p->S);
+        if ((long long)p->W * p->O * 3 * p->S + 2 * p->S > 65535)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 3: tap table too large for 16-bit offsets");
+        if (p->batch < 4 || (p->batch & (p->batch - 1)) != 0)
+            return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two >= 4", p->batch);
+        if (p->chunk < 1) return fail(GRID_ERR_UNSUPPORTED, "chunk %d must be positive", p->chunk);
+        if (p->threads % 32 != 0 || p->threads < 32 || p->threads > 1024)
+            return fail(GRID_ERR_UNSUPPORTED, "threads_per_cta %d must be a multiple of 32 in [32, 1024]", p->threads);
+        int threads = p->threads < d.max_threads ? p->threads : d.max_threads;
+        if (threads < d.gt)
+            return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA may have %d", d.gt, threads);
+        p->bin_u = p->bin_v = p->S;
+        p->row_u = p->row_v = 3 * p->S;
+        p->nbx = p->S / p->cu;
+        p->nby = p->S / p->cv;
+        p->team_threads = d.team;
+        int groups = threads / d.gt;
+        if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
+        const size_t taps = ((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15;
+        const size_t per_group = d.group_bytes(p->batch);
+        if (taps + per_group > (size_t)p->max_smem)
+            return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one group's buffers (%zu B) exceed %d B of shared memory",
+                        taps, per_group, p->max_smem);
+        const size_t fit = ((size_t)p->max_smem - taps) / per_group;
+        if ((size_t)groups > fit) groups = (int)fit;
+        p->groups_per_cta = groups;
+        p->threads = groups * d.gt;
+        p->teams_per_cta = groups * d.tpg;
+        p->queue_teams = d.tpg;
+        p->ctas_per_sm = 1;
+        p->smem_bytes = (int)(taps + (size_t)groups * per_group);
         return GRID_OK;
     }
     if (p->variant == 2) {
@@ -198,7 +278,9 @@ void default_tuning(grid_plan* p) {
     const int logs = log2_exact(p->S);
     if (logs >= 2 && logs <= 5) {
         grid_plan trial = *p;
-        trial.variant = 2;
+        trial.variant = 3;
+        trial.threads = 1024;              // clipped to the kernel's register-limited maximum
+        trial.batch = 32;
         if (trial.P >= 4) { trial.cu = 2; trial.cv = 2; }
         else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = 2; }
         else { trial.cu = 4; trial.cv = (logs >= 3) ? 4 : 2; }
@@ -210,7 +292,7 @@ void default_tuning(grid_plan* p) {
 
 QuantParams quant_params(const grid_plan* p) {
     QuantParams q;
-    q.format = p->variant == 2 ? 1 : 0;
+    q.format = p->variant >= 2 ? 1 : 0;
     q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
     q.oversample = p->O;
     q.shift = p->O - (p->O * p->S + 1) / 2;
@@ -299,7 +381,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     if (batch > 0) trial.batch = batch;
     if (chunk > 0) trial.chunk = chunk;
     if (ctas_per_sm > 0) trial.ctas_per_sm = ctas_per_sm;
-    if (trial.variant < 0 || trial.variant > 2)
+    if (trial.variant < 0 || trial.variant > 3)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: unknown variant %d", trial.variant);
     const int rc = derive(&trial);
     if (rc != GRID_OK) return rc;
@@ -408,16 +490,19 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         while ((1 << shift) < plan->batch) ++shift;
         gp.batch_shift = shift;
         // adaptive chunk length for small inputs: keep every SM busy
-        long long want_groups = (long long)plan->n_sm * plan->ctas_per_sm * 4;
-        long long per_group = (long long)plan->teams_per_cta * plan->chunk;
+        const int qt = plan->variant == 3 ? plan->queue_teams : plan->teams_per_cta;   // teams per queue entry
+        const int queues = plan->variant == 3 ? plan->groups_per_cta : 1;               // queue consumers per CTA
+        long long want_groups = (long long)plan->n_sm * plan->ctas_per_sm * queues * 4;
+        long long per_group = (long long)qt * plan->chunk;
         if ((plan->n_vis + per_group - 1) / per_group < want_groups) {
-            long long chunk = plan->n_vis / (want_groups * plan->teams_per_cta);
+            long long chunk = plan->n_vis / (want_groups * qt);
             chunk = (chunk + plan->batch - 1) / plan->batch * plan->batch;
             if (chunk < plan->batch) chunk = plan->batch;
             if (chunk < gp.chunk) gp.chunk = (int)chunk;
-            per_group = (long long)plan->teams_per_cta * gp.chunk;
+            per_group = (long long)qt * gp.chunk;
         }
         gp.n_groups_a = (plan->n_vis + per_group - 1) / per_group;
+        gp.groups_per_cta = plan->groups_per_cta;
         // time-innermost decomposition: chunk = tc time steps x all channels of one baseline
         gp.hop_stats = hop_stats;
         gp.force_mode = have_layout ? plan->traversal : 0;
@@ -431,17 +516,20 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
             gp.cb_shift = shift - tshift;
             gp.n_tblocks = (n_times + tc - 1) / tc;
             gp.n_chunks_b = (long long)plan->n_baselines * gp.n_tblocks;
-            gp.n_groups_b = (gp.n_chunks_b + plan->teams_per_cta - 1) / plan->teams_per_cta;
+            gp.n_groups_b = (gp.n_chunks_b + qt - 1) / qt;
         } else {
             gp.tc = 1; gp.n_tblocks = 1;
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
-        kernel_fn fn = plan->variant == 2 ? lookup_cyclic(plan->cu, plan->cv, plan->P, log2_exact(plan->S))
+        const int logs = log2_exact(plan->S);
+        kernel_fn fn = plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs).fn
+                     : plan->variant == 2 ? lookup_cyclic(plan->cu, plan->cv, plan->P, logs)
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan->smem_bytes);
         if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         long long ctas = (long long)plan->n_sm * plan->ctas_per_sm;
-        if (ctas > max_groups) ctas = max_groups;
+        const long long need = (max_groups + queues - 1) / queues;
+        if (ctas > need) ctas = need;
         fn<<<(unsigned)ctas, plan->threads, plan->smem_bytes, stream>>>(gp);
         plan->last_launches++;
     }

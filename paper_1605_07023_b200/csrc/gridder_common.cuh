@@ -44,6 +44,7 @@ struct GridParams {
     int N, S, n_rows;         // n_rows = W*O
     int bin_u, bin_v, row_u, row_v, nbx, nby;
     int team_threads, teams_per_cta, batch, chunk, batch_shift;
+    int groups_per_cta;       // variant 3: warp groups per CTA (each its own queue consumer)
     // layout hint (0 = unknown) and time-innermost traversal: a mode-1 chunk is tc time steps x all
     // channels of one baseline; a batch is tc x (1 << cb_shift) samples
     int n_chan, n_times, tc, cb_shift, n_tblocks;

@@ -116,6 +116,31 @@ def test_every_cyclic_block(oracle_mod, cu, cv, P, S):
     assert_parity(got, ref, f"cyclic C={cu}x{cv} P={P} S={S}")
 
 
+WARP = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (1, 1, 2), (2, 2, 2), (4, 2, 2), (4, 4, 2),
+        (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 2, 4)]
+
+
+@pytest.mark.parametrize("cu,cv,P", WARP)
+@pytest.mark.parametrize("S", [4, 8, 16, 32])
+def test_every_warp_block(oracle_mod, cu, cv, P, S):
+    # warp-autonomous kernel (variant 3): teams of 1..1024 threads (several teams per warp up to a
+    # whole CTA per team), ragged tail, samples off the grid, jumps larger than the support, 3 planes
+    if cu > S or cv > S:
+        pytest.skip("block larger than the support")
+    N, O, W, n = 128, 4, 3, 20_003
+    uvw, vis, wts, kernel = synth.random_problem(2000 + 100 * cu + 10 * cv + P + S, n, N, S, O, W, P,
+                                                 spread=0.5, walk=1.5)
+    uvw[5000:5100, :2] = np.random.default_rng(S).uniform(-60, 60, (100, 2))    # big jumps
+    uvw[7000:7010, 0] = np.nan
+    vis[7000:7010] = np.inf
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    for batch, chunk in ((32, 300), (8, 64)):
+        got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                            tuning=dict(variant=3, cu=cu, cv=cv, threads_per_cta=1024, batch=batch, chunk=chunk))
+        assert (info["variant"], info["cu"], info["cv"], info["bin_u"]) == (3, cu, cv, S)
+        assert_parity(got, ref, f"warp C={cu}x{cv} P={P} S={S} batch={batch} {info}")
+
+
 @pytest.mark.parametrize("S,P,cu,cv", [(1, 1, 1, 1), (2, 4, 2, 1), (3, 1, 2, 2), (4, 1, 4, 2), (5, 2, 2, 2),
                                        (16, 1, 4, 4), (16, 4, 2, 2), (32, 1, 8, 4), (32, 4, 4, 2), (13, 1, 4, 4)])
 def test_supports(oracle_mod, S, P, cu, cv):

@@ -29,9 +29,10 @@ namespace gridb200 {
 
 struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
     long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)
-    int len;                  // mode 0: positions in the chunk
+    int len;                  // mode 0: positions in the chunk; mode 1: channels in the chunk
     int h;                    // mode 1: time steps in this block (0: empty chunk)
-    int col0, rowpar;         // mode 0 with layout: column of `base` and parity of its time row
+    int col0, rowpar;         // mode 0 with layout: column of `base` and parity of its time row;
+                              // mode 1: first channel of the chunk
     int pad0, pad1;
 };
 
@@ -150,6 +151,29 @@ grid_warp_kernel(const GridParams gp) {
         for (int q = 0; q < P; ++q) v[q] = make_float2(0.f, 0.f);
     };
 
+    // Same, but the atomic adds are predicated: used in the row pass for points whose column has
+    // just been flushed (their accumulators are zero; skipping saves the L2 traffic, not a branch).
+    auto flush_point_if = [&](float2 (&v)[P], uint32_t cell, uint32_t skip) {
+        float* p = gp.grid + (size_t)cell * (2 * P);
+        if constexpr (P == 4) {
+            asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %9, 0;\n\t"
+                         "@q red.relaxed.gpu.global.add.v4.f32 [%8], {%0, %1, %2, %3};\n\t"
+                         "@q red.relaxed.gpu.global.add.v4.f32 [%8+16], {%4, %5, %6, %7};\n\t}"
+                         :: "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y),
+                            "f"(v[3].x), "f"(v[3].y), "l"(p), "r"(skip) : "memory");
+        } else if constexpr (P == 2) {
+            asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %5, 0;\n\t"
+                         "@q red.relaxed.gpu.global.add.v4.f32 [%4], {%0, %1, %2, %3};\n\t}"
+                         :: "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "l"(p), "r"(skip) : "memory");
+        } else {
+            asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %3, 0;\n\t"
+                         "@q red.relaxed.gpu.global.add.v2.f32 [%2], {%0, %1};\n\t}"
+                         :: "f"(v[0].x), "f"(v[0].y), "l"(p), "r"(skip) : "memory");
+        }
+#pragma unroll
+        for (int q = 0; q < P; ++q) v[q] = make_float2(0.f, 0.f);
+    };
+
     int mode = gp.force_mode;
     if (mode < 0) {
         mode = 0;
@@ -161,7 +185,7 @@ grid_warp_kernel(const GridParams gp) {
         }
     }
     const long long n_groups = mode ? gp.n_groups_b : gp.n_groups_a;
-    const int n_batches = mode ? (gp.n_chan + (1 << gp.cb_shift) - 1) >> gp.cb_shift
+    const int n_batches = mode ? (gp.chunk_cols + (1 << gp.cb_shift) - 1) >> gp.cb_shift
                                : (gp.chunk + B - 1) >> bshift;
 
     // a9: take the next chunk group from the queue; lanes t < TPG work out their team's geometry
@@ -190,10 +214,15 @@ grid_warp_kernel(const GridParams gp) {
                     cg.rowpar = (int)(row & 1);
                 }
             } else if (chunk_id < gp.n_chunks_b) {
-                const long long bl = chunk_id / gp.n_tblocks;
-                const int tb = (int)(chunk_id - bl * gp.n_tblocks);
+                // chunk = (baseline, block of tc time steps, block of chunk_cols channels)
+                const long long per_bl = (long long)gp.n_tblocks * gp.n_cblocks;
+                const long long bl = chunk_id / per_bl;
+                const int rem = (int)(chunk_id - bl * per_bl);
+                const int tb = rem / gp.n_cblocks, cc = rem - tb * gp.n_cblocks;
                 cg.h = gp.n_times - tb * gp.tc < gp.tc ? gp.n_times - tb * gp.tc : gp.tc;
                 cg.base = (bl * gp.n_times + (long long)tb * gp.tc) * gp.n_chan;
+                cg.col0 = cc * gp.chunk_cols;
+                cg.len = gp.n_chan - cg.col0 < gp.chunk_cols ? gp.n_chan - cg.col0 : gp.chunk_cols;
             }
             geom[par * TPG + lg] = cg;
         }
@@ -206,7 +235,7 @@ grid_warp_kernel(const GridParams gp) {
             const int left = cg.len - (b << bshift);
             return left < 0 ? 0 : (left < B ? left : B);
         }
-        int cols = gp.n_chan - (b << gp.cb_shift);
+        int cols = cg.len - (b << gp.cb_shift);
         if (cols > (1 << gp.cb_shift)) cols = 1 << gp.cb_shift;
         return cols < 0 ? 0 : cols * cg.h;
     };
@@ -224,7 +253,7 @@ grid_warp_kernel(const GridParams gp) {
             return a;
         }
         const int ci = (int)((uint32_t)k / (uint32_t)cg.h), tt = k - ci * cg.h;
-        const int col = (b << gp.cb_shift) + ci;
+        const int col = cg.col0 + (b << gp.cb_shift) + ci;
         const int ti = (col & 1) ? cg.h - 1 - tt : tt;
         return cg.base + (long long)ti * gp.n_chan + col;
     };
@@ -327,8 +356,12 @@ grid_warp_kernel(const GridParams gp) {
             }
             if constexpr (TPG > 1) cnt = __reduce_max_sync(0xffffffffu, cnt);
 
+            const uint4* rp = my_rec;
+            const float2* vp = my_vis;
+            uint4 c_next = *rp;
             for (int s = 0; s < cnt; ++s) {
-                const uint4 c = my_rec[s];
+                const uint4 c = c_next;
+                c_next = *++rp;                        // next record (one slot of slack follows the batch)
                 bool moved;
                 if constexpr (WIDE) moved = ((c.z & MX) | (c.w & MY)) != 0;
                 else moved = (c.w & MXY) != 0;
@@ -349,7 +382,7 @@ grid_warp_kernel(const GridParams gp) {
                         if (mys & (1u << (bb * DV))) { // owned row bb left the footprint
 #pragma unroll
                             for (int a = 0; a < CU; ++a)
-                                if (!(mxs & (1u << (a * DU)))) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                                flush_point_if(acc[bb][a], ry[bb] + (uint32_t)cx[a], mxs & (1u << (a * DU)));
                             ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
                         }
                     }
@@ -369,16 +402,17 @@ grid_warp_kernel(const GridParams gp) {
 #pragma unroll
                 for (int bb = 0; bb < CV; ++bb) gv[bb] = tv[bb * DV];
                 if constexpr (P == 4) {
-                    const float4 v01 = *reinterpret_cast<const float4*>(my_vis + s * 4);
-                    const float4 v23 = *reinterpret_cast<const float4*>(my_vis + s * 4 + 2);
+                    const float4 v01 = *reinterpret_cast<const float4*>(vp);
+                    const float4 v23 = *reinterpret_cast<const float4*>(vp + 2);
                     v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
                     v[2] = make_float2(v23.x, v23.y); v[3] = make_float2(v23.z, v23.w);
                 } else if constexpr (P == 2) {
-                    const float4 v01 = *reinterpret_cast<const float4*>(my_vis + s * 2);
+                    const float4 v01 = *reinterpret_cast<const float4*>(vp);
                     v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
                 } else {
-                    v[0] = my_vis[s];
+                    v[0] = *vp;
                 }
+                vp += P;
                 if constexpr (P < CU) {
                     // a6 reordered: T = Gv_j * V_p first, then Gu_i * T
 #pragma unroll

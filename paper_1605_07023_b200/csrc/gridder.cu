@@ -281,6 +281,7 @@ void default_tuning(grid_plan* p) {
         trial.variant = 3;
         trial.threads = 1024;              // clipped to the kernel's register-limited maximum
         trial.batch = 32;
+        trial.chunk = 256;
         if (trial.P >= 4) { trial.cu = 2; trial.cv = 2; }
         else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = 2; }
         else { trial.cu = 4; trial.cv = (logs >= 3) ? 4 : 2; }
@@ -515,7 +516,17 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
             gp.tc = tc;
             gp.cb_shift = shift - tshift;
             gp.n_tblocks = (n_times + tc - 1) / tc;
-            gp.n_chunks_b = (long long)plan->n_baselines * gp.n_tblocks;
+            gp.n_cblocks = 1;
+            gp.chunk_cols = n_chan;
+            if (plan->variant == 3) {      // chunk = tc time steps x chunk_cols channels ~ gp.chunk samples
+                const int cpb = 1 << gp.cb_shift;
+                int cols = (gp.chunk / tc + cpb - 1) / cpb * cpb;
+                if (cols < cpb) cols = cpb;
+                if (cols > n_chan) cols = (n_chan + cpb - 1) / cpb * cpb;
+                gp.chunk_cols = cols;
+                gp.n_cblocks = (n_chan + cols - 1) / cols;
+            }
+            gp.n_chunks_b = (long long)plan->n_baselines * gp.n_tblocks * gp.n_cblocks;
             gp.n_groups_b = (gp.n_chunks_b + qt - 1) / qt;
         } else {
             gp.tc = 1; gp.n_tblocks = 1;

@@ -155,6 +155,16 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def ncu_traffic(workload):
+    """DRAM bytes per launch of the gridding kernel (dram__bytes_read.sum + dram__bytes_write.sum) from
+    the committed `ncu --set full` capture of this workload (profiles/ncu_traffic.json), else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+    except (OSError, ValueError):
+        return None
+
+
 def parse_tuning(text):
     out = {}
     for item in filter(None, text.split(",")):
@@ -217,6 +227,9 @@ def run_ours(args):
         plan.set_tuning(**tuning)
     plan.allocate_workspace(dev)
     info = plan.info()
+    kernel_name = {0: "grid_scatter_kernel", 1: "grid_coarsened_kernel", 2: "grid_cyclic_kernel",
+                   3: "grid_warp_kernel"}[info["variant"]]
+    kernel_name += "<%d,%d,%d>" % (info["cu"], info["cv"], P)
 
     # number of valid samples (for the metric) from the library's own quantise pass
     q = plan.quantise(d_uvw)
@@ -298,8 +311,8 @@ def run_ours(args):
                        "tuning": info},
             "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / PEAK_FP32_TFLOPS, "traffic": None,
-                         "kernel": "grid_coarsened_kernel", "kernel_ms": kernel_ms,
+                         "frac": achieved / PEAK_FP32_TFLOPS, "traffic": ncu_traffic(cfg.name),
+                         "kernel": kernel_name, "kernel_ms": kernel_ms,
                          "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (derived; DESIGN.md)"},
             "clocks": clocks, "gpu_launches": launches,
         }

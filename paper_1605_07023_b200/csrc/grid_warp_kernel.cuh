@@ -136,9 +136,14 @@ grid_warp_kernel(const GridParams gp) {
 #pragma unroll
     for (int b = 0; b < CV; ++b) ry[b] = 0;
 
+    // the grid pointer lives in registers: reloading it from the constant bank inside the divergent
+    // flush sections showed up as long-scoreboard stalls (profiles/)
+    float* gridp = gp.grid;
+    asm volatile("" : "+l"(gridp));
+
     // a8: one grid point, all polarisations: atomic add, then clear
     auto flush_point = [&](float2 (&v)[P], uint32_t cell) {
-        float* p = gp.grid + (size_t)cell * (2 * P);
+        float* p = gridp + (size_t)cell * (2 * P);
         if constexpr (P == 4) {
             red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
             red_add_v4(p + 4, v[2].x, v[2].y, v[3].x, v[3].y);
@@ -154,7 +159,7 @@ grid_warp_kernel(const GridParams gp) {
     // Same, but the atomic adds are predicated: used in the row pass for points whose column has
     // just been flushed (their accumulators are zero; skipping saves the L2 traffic, not a branch).
     auto flush_point_if = [&](float2 (&v)[P], uint32_t cell, uint32_t skip) {
-        float* p = gp.grid + (size_t)cell * (2 * P);
+        float* p = gridp + (size_t)cell * (2 * P);
         if constexpr (P == 4) {
             asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %9, 0;\n\t"
                          "@q red.relaxed.gpu.global.add.v4.f32 [%8], {%0, %1, %2, %3};\n\t"

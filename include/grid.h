@@ -79,15 +79,17 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
 int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid_stream_t stream);
 
 /* Override the tuned launch configuration (autotuning).  Any argument <= 0 keeps the
- * current value.  variant: 2 = coarsened kernel with bin == support (power-of-two supports 4..32;
- * default for those), 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any
+ * current value.  variant: 3 = warp-autonomous coarsened kernel with bin == support (power-of-two
+ * supports 4..32; default for those), 2 = its CTA-synchronous predecessor, 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any
  * support; default otherwise), 0 = naive scatter (one atomic per update; diagnostic baseline only).
  *   cu, cv            coarsening block per thread (u, v), each in {1,2,4,8}, cu*cv*n_pol <= 32
  *   threads_per_cta   multiple of 32, <= 1024
  *   batch             samples staged to shared memory per team per step
  *   chunk             samples a team grids before its final flush (1024)
  *   ctas_per_sm       persistent CTAs per SM
- * Returns GRID_ERR_UNSUPPORTED if the combination does not fit (shared memory, registers). */
+ * A block that is not instantiated for the plan's current polarisation split (grid_plan_set_pol_split)
+ * resets the split to 1.  Returns GRID_ERR_UNSUPPORTED if the combination does not fit (shared
+ * memory, registers). */
 int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threads_per_cta,
                          int batch, int chunk, int ctas_per_sm);
 
@@ -99,8 +101,22 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
  * on "the coordinates and ordering of the data". */
 int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block);
 
-/* HOST out[16]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
- * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, 0. */
+/* Order in which chunks enter the work queue (PAPER.md:103 fixes the chunks, not their order; the
+ * result is the same sum): 1 = sorted by the coarse grid tile of the chunk's first sample, so that
+ * chunks in flight together flush to neighbouring grid cells (three extra small launches per
+ * grid_execute), 0 = input (baseline) order, -1 = sorted only when the grid exceeds 256 MB, i.e. twice
+ * the L2 (default).  Power-of-two supports (variant 3) only; ignored otherwise. */
+int grid_plan_set_chunk_order(grid_plan* plan, int mode);
+
+/* Variant 3, n_pol = 4: spread the polarisations of one grid point over `lanes` adjacent threads
+ * (1 or 2).  With 2, the two 16-byte atomics of a 32-byte grid point leave in one instruction and
+ * cost the L2 one sector operation instead of two.  Set the block (cu, cv) first; returns
+ * GRID_ERR_UNSUPPORTED if that combination is not instantiated. */
+int grid_plan_set_pol_split(grid_plan* plan, int lanes);
+
+/* HOST out[20]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
+ * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, chunk order mode,
+ * polarisation split, warp groups per CTA, 0, 0. */
 int grid_plan_get_info(const grid_plan* plan, int* out);
 
 /* Measurement hook: two caller-owned cudaEvent_t (passed as void*) that the following grid_execute

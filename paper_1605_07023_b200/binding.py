@@ -16,7 +16,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
     "grid_plan_set_workspace", "grid_execute", "grid_quantise", "grid_plan_set_tuning",
-    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
+    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -39,6 +39,8 @@ _lib.grid_plan_set_tuning.argtypes = [_vp] + [_int] * 7
 _lib.grid_plan_get_info.argtypes = [_vp, _vp]
 _lib.grid_plan_set_traversal.argtypes = [_vp, _int, _int]
 _lib.grid_plan_set_kernel_events.argtypes = [_vp, _vp, _vp]
+_lib.grid_plan_set_chunk_order.argtypes = [_vp, _int]
+_lib.grid_plan_set_pol_split.argtypes = [_vp, _int]
 _lib.grid_plan_last_launches.argtypes = [_vp]
 _lib.grid_plan_destroy.argtypes = [_vp]
 _lib.grid_plan_destroy.restype = None
@@ -77,7 +79,7 @@ def _stream(stream):
 
 
 INFO_FIELDS = ("variant", "cu", "cv", "bin_u", "bin_v", "team_threads", "teams_per_cta",
-               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block")
+               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block", "chunk_order", "pol_split", "groups_per_cta")
 
 
 class GridPlan:
@@ -127,8 +129,14 @@ class GridPlan:
     def set_traversal(self, mode=-1, time_block=0):
         _check(_lib.grid_plan_set_traversal(self._h, mode, time_block), "grid_plan_set_traversal")
 
+    def set_pol_split(self, lanes=1):
+        _check(_lib.grid_plan_set_pol_split(self._h, lanes), "grid_plan_set_pol_split")
+
+    def set_chunk_order(self, mode=-1):
+        _check(_lib.grid_plan_set_chunk_order(self._h, mode), "grid_plan_set_chunk_order")
+
     def info(self) -> dict:
-        out = (ctypes.c_int * 16)()
+        out = (ctypes.c_int * 20)()
         _check(_lib.grid_plan_get_info(self._h, out), "grid_plan_get_info")
         return dict(zip(INFO_FIELDS, list(out)))
 
@@ -184,6 +192,10 @@ def grid_visibilities(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis
             tuning = dict(tuning)
             if "traversal" in tuning or "time_block" in tuning:
                 plan.set_traversal(tuning.pop("traversal", -1), tuning.pop("time_block", 0))
+            if "chunk_order" in tuning:
+                plan.set_chunk_order(tuning.pop("chunk_order"))
+            if "pol_split" in tuning:          # before the block: (cu, cv) is validated against it
+                plan.set_pol_split(tuning.pop("pol_split"))
             if tuning:
                 plan.set_tuning(**tuning)
         plan.allocate_workspace(uvw.device)

@@ -24,6 +24,7 @@
 #pragma once
 #include "gridder_common.cuh"
 #include "grid_cyclic_kernel.cuh"      // moved_mask<>, flush helpers
+#include "chunk_order.cuh"
 
 namespace gridb200 {
 
@@ -48,15 +49,21 @@ __device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int CU, int CV, int P, int LOGS>
+// PS ("polarisation split"): the P polarisations of a grid point are divided over PS adjacent lanes,
+// each holding PT = P/PS of them.  With P = 4, PS = 2 the two 16-byte atomics that make up one
+// 32-byte grid point come from neighbouring lanes of ONE instruction and reach the L2 as one sector
+// operation instead of two -- the L2's atomic sector rate is the second bound of this kernel.
+template <int CU, int CV, int P, int LOGS, int PS = 1>
 struct WarpKernelTraits {
+    static_assert(P % PS == 0, "polarisations must divide evenly over the split");
     static constexpr int S = 1 << LOGS;
+    static constexpr int PT = P / PS;                     // polarisations per thread
     static constexpr int DU = S / CU, DV = S / CV;       // spacing of a thread's owned positions
-    static constexpr int TEAM = DU * DV;                  // threads per bin
+    static constexpr int TEAM = DU * DV * PS;             // threads per bin
     static constexpr int GW = TEAM > 32 ? TEAM / 32 : 1;  // warps per group
     static constexpr int GT = GW * 32;                    // threads per group
     static constexpr int TPG = TEAM >= 32 ? 1 : 32 / TEAM;    // teams (chunks in flight) per group
-    static constexpr int ACC = 2 * CU * CV * P;
+    static constexpr int ACC = 2 * CU * CV * PT;
     static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
     // shared memory of one group for a batch of B samples per team
     __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + 8 * P); }
@@ -67,18 +74,22 @@ struct WarpKernelTraits {
     }
 };
 
-template <int CU, int CV, int P, int LOGS>
-__global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS>::MAX_THREADS), 1)
+template <int CU, int CV, int P, int LOGS, int PS = 1>
+__global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS, PS>::MAX_THREADS), 1)
 grid_warp_kernel(const GridParams gp) {
-    using T = WarpKernelTraits<CU, CV, P, LOGS>;
+    using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
+    constexpr int PT = T::PT;
     constexpr int S = T::S, DU = T::DU, DV = T::DV, TEAM = T::TEAM, GW = T::GW, GT = T::GT, TPG = T::TPG;
     constexpr int ROW = 3 * S;                         // tripled tap row: k[t mod S], t < 3S
     constexpr bool WIDE = S > 16;                      // record format: 32-bit masks need two words
     static_assert(CU <= S && CV <= S, "block larger than the support");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* taps = reinterpret_cast<float2*>(smem_raw);
-    const size_t taps_bytes = ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
+    // [0, 16): zeros.  Accumulators are cleared with one LDS.128 from here instead of four moves: the
+    // moves ptxas emits (IMAD.U32 Rx, RZ, RZ, URy) occupy the FMA pipe the kernel is short of.
+    const uint32_t zero_addr = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    float2* taps = reinterpret_cast<float2*>(smem_raw + 16);
+    const size_t taps_bytes = 16 + (((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15);
     const int B = gp.batch, bshift = gp.batch_shift;
     const int slots = TPG * B;
 
@@ -94,6 +105,7 @@ grid_warp_kernel(const GridParams gp) {
     uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
     uint32_t* ctrl = last_pos + 2 * TPG;
 
+    if (tid < 4) reinterpret_cast<float*>(smem_raw)[tid] = 0.f;
     for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {          // a4
         const int r = k / ROW, t = (k - r * ROW) & (S - 1);
         taps[k] = __ldg(gp.kern + (size_t)r * S + t);
@@ -109,7 +121,8 @@ grid_warp_kernel(const GridParams gp) {
     // a5: ownership
     const int tg = (TPG > 1) ? lg / TEAM : 0;          // my team within the group
     const int lt = lg - tg * TEAM;
-    const int r0 = lt % DU, s0 = lt / DU;
+    const int half = lt % PS, ct = lt / PS;            // my share of the polarisations; my block owner index
+    const int r0 = ct % DU, s0 = ct / DU;
     uint32_t MX = 0, MY = 0;
 #pragma unroll
     for (int a = 0; a < CU; ++a) MX |= 1u << (r0 + a * DU);
@@ -117,18 +130,18 @@ grid_warp_kernel(const GridParams gp) {
     for (int b = 0; b < CV; ++b) MY |= 1u << (s0 + b * DV);
     const uint32_t MXY = MX | (MY << 16);              // !WIDE: both masks in one word
     const uint4* my_rec = crec + (size_t)tg * B;
-    const float2* my_vis = cvis + (size_t)tg * B * P;
+    const float2* my_vis = cvis + (size_t)tg * B * P + half * PT;
     const unsigned char* my_tu = reinterpret_cast<const unsigned char*>(taps + r0);
     const unsigned char* my_tv = reinterpret_cast<const unsigned char*>(taps + s0);
     const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
 
-    float2 acc[CV][CU][P];
+    float2 acc[CV][CU][PT];
 #pragma unroll
     for (int b = 0; b < CV; ++b)
 #pragma unroll
         for (int a = 0; a < CU; ++a)
 #pragma unroll
-            for (int q = 0; q < P; ++q) acc[b][a][q] = make_float2(0.f, 0.f);
+            for (int q = 0; q < PT; ++q) acc[b][a][q] = make_float2(0.f, 0.f);
     int cx[CU];                     // x of the grid point currently held for owned column a
     uint32_t ry[CV];                // y * N of the grid point currently held for owned row b
 #pragma unroll
@@ -141,32 +154,44 @@ grid_warp_kernel(const GridParams gp) {
     float* gridp = gp.grid;
     asm volatile("" : "+l"(gridp));
 
+    auto clear_point = [&](float2 (&v)[PT]) {
+        if constexpr (PT == 4) {
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%8];\n\tld.shared.v4.f32 {%4, %5, %6, %7}, [%8];"
+                         : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y),
+                           "=f"(v[3].x), "=f"(v[3].y) : "r"(zero_addr));
+        } else if constexpr (PT == 2) {
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y) : "r"(zero_addr));
+        } else {
+            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v[0].x), "=f"(v[0].y) : "r"(zero_addr));
+        }
+    };
+
     // a8: one grid point, all polarisations: atomic add, then clear
-    auto flush_point = [&](float2 (&v)[P], uint32_t cell) {
-        float* p = gridp + (size_t)cell * (2 * P);
-        if constexpr (P == 4) {
+    auto flush_point = [&](float2 (&v)[PT], uint32_t cell) {
+        float* p = gridp + (size_t)cell * (2 * P) + half * (2 * PT);
+        if constexpr (PT == 4) {
             red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
             red_add_v4(p + 4, v[2].x, v[2].y, v[3].x, v[3].y);
-        } else if constexpr (P == 2) {
+        } else if constexpr (PT == 2) {
             red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
         } else {
             red_add_v2(p, v[0].x, v[0].y);
         }
-#pragma unroll
-        for (int q = 0; q < P; ++q) v[q] = make_float2(0.f, 0.f);
+        clear_point(v);
     };
 
     // Same, but the atomic adds are predicated: used in the row pass for points whose column has
     // just been flushed (their accumulators are zero; skipping saves the L2 traffic, not a branch).
-    auto flush_point_if = [&](float2 (&v)[P], uint32_t cell, uint32_t skip) {
-        float* p = gridp + (size_t)cell * (2 * P);
-        if constexpr (P == 4) {
+    auto flush_point_if = [&](float2 (&v)[PT], uint32_t cell, uint32_t skip) {
+        float* p = gridp + (size_t)cell * (2 * P) + half * (2 * PT);
+        if constexpr (PT == 4) {
             asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %9, 0;\n\t"
                          "@q red.relaxed.gpu.global.add.v4.f32 [%8], {%0, %1, %2, %3};\n\t"
                          "@q red.relaxed.gpu.global.add.v4.f32 [%8+16], {%4, %5, %6, %7};\n\t}"
                          :: "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y),
                             "f"(v[3].x), "f"(v[3].y), "l"(p), "r"(skip) : "memory");
-        } else if constexpr (P == 2) {
+        } else if constexpr (PT == 2) {
             asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %5, 0;\n\t"
                          "@q red.relaxed.gpu.global.add.v4.f32 [%4], {%0, %1, %2, %3};\n\t}"
                          :: "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "l"(p), "r"(skip) : "memory");
@@ -175,20 +200,10 @@ grid_warp_kernel(const GridParams gp) {
                          "@q red.relaxed.gpu.global.add.v2.f32 [%2], {%0, %1};\n\t}"
                          :: "f"(v[0].x), "f"(v[0].y), "l"(p), "r"(skip) : "memory");
         }
-#pragma unroll
-        for (int q = 0; q < P; ++q) v[q] = make_float2(0.f, 0.f);
+        clear_point(v);
     };
 
-    int mode = gp.force_mode;
-    if (mode < 0) {
-        mode = 0;
-        if (gp.n_chan > 0) {
-            const float hc = __ldg(gp.hop_stats), ht = __ldg(gp.hop_stats + 1);
-            const float cost0 = ((gp.n_chan - 1) * hc + ht) / gp.n_chan;
-            const float cost1 = ((gp.tc - 1) * ht + hc) / gp.tc;
-            mode = cost1 < cost0 ? 1 : 0;
-        }
-    }
+    const int mode = pick_mode(gp);
     const long long n_groups = mode ? gp.n_groups_b : gp.n_groups_a;
     const int n_batches = mode ? (gp.chunk_cols + (1 << gp.cb_shift) - 1) >> gp.cb_shift
                                : (gp.chunk + B - 1) >> bshift;
@@ -206,10 +221,16 @@ grid_warp_kernel(const GridParams gp) {
         }
         const long long g = v;
         if (g < n_groups && lg < TPG) {
-            const long long chunk_id = g * TPG + lg;
+            long long chunk_id = g * TPG + lg;
+            bool have = true;
+            if (gp.order) {                            // locality-sorted queue (chunk_order.cuh)
+                have = chunk_id < chunk_count(gp, mode);
+                if (have) chunk_id = __ldg(gp.order + chunk_id);
+            }
             WarpChunk cg;
             cg.base = 0; cg.len = 0; cg.h = 0; cg.col0 = 0; cg.rowpar = 0; cg.pad0 = cg.pad1 = 0;
-            if (mode == 0) {
+            if (!have) {
+            } else if (mode == 0) {
                 cg.base = chunk_id * gp.chunk;
                 const long long left = gp.n_vis - cg.base;
                 cg.len = left <= 0 ? 0 : (left < gp.chunk ? (int)left : gp.chunk);
@@ -370,6 +391,9 @@ grid_warp_kernel(const GridParams gp) {
                 bool moved;
                 if constexpr (WIDE) moved = ((c.z & MX) | (c.w & MY)) != 0;
                 else moved = (c.w & MXY) != 0;
+#ifdef GRIDB200_PROBE_NO_FLUSH                             /* measurement probe only (wrong results) */
+                moved = false;
+#endif
                 if (moved) {                           // a5/a8: some of my points moved
                     const int i0 = (int)(c.x & 0x7fffu), j0 = (int)(c.x >> 16);
                     const uint32_t mxs = (WIDE ? c.z : c.w) >> r0;
@@ -401,29 +425,32 @@ grid_warp_kernel(const GridParams gp) {
                     tu = reinterpret_cast<const float2*>(my_tu + c.y);
                     tv = reinterpret_cast<const float2*>(my_tv + c.z);
                 }
-                float2 gu[CU], gv[CV], v[P];
+                float2 gu[CU], gv[CV], v[PT];
 #pragma unroll
                 for (int a = 0; a < CU; ++a) gu[a] = tu[a * DU];
 #pragma unroll
                 for (int bb = 0; bb < CV; ++bb) gv[bb] = tv[bb * DV];
-                if constexpr (P == 4) {
+                if constexpr (PT == 4) {
                     const float4 v01 = *reinterpret_cast<const float4*>(vp);
                     const float4 v23 = *reinterpret_cast<const float4*>(vp + 2);
                     v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
                     v[2] = make_float2(v23.x, v23.y); v[3] = make_float2(v23.z, v23.w);
-                } else if constexpr (P == 2) {
+                } else if constexpr (PT == 2) {
                     const float4 v01 = *reinterpret_cast<const float4*>(vp);
                     v[0] = make_float2(v01.x, v01.y); v[1] = make_float2(v01.z, v01.w);
                 } else {
                     v[0] = *vp;
                 }
                 vp += P;
-                if constexpr (P < CU) {
+#ifdef GRIDB200_PROBE_NO_MAC                               /* measurement probe only (wrong results) */
+                if (gu[0].x == 12345.678f)
+#endif
+                if constexpr (PT < CU) {
                     // a6 reordered: T = Gv_j * V_p first, then Gu_i * T
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb) {
 #pragma unroll
-                        for (int q = 0; q < P; ++q) {
+                        for (int q = 0; q < PT; ++q) {
                             const float tr = gv[bb].x * v[q].x - gv[bb].y * v[q].y;
                             const float ti = gv[bb].x * v[q].y + gv[bb].y * v[q].x;
 #pragma unroll
@@ -443,7 +470,7 @@ grid_warp_kernel(const GridParams gp) {
                             const float gr = gv[bb].x * gu[a].x - gv[bb].y * gu[a].y;       // a6
                             const float gi = gv[bb].x * gu[a].y + gv[bb].y * gu[a].x;
 #pragma unroll
-                            for (int q = 0; q < P; ++q) {                                    // a7
+                            for (int q = 0; q < PT; ++q) {                                   // a7
                                 acc[bb][a][q].x = fmaf(gr, v[q].x, acc[bb][a][q].x);
                                 acc[bb][a][q].x = fmaf(-gi, v[q].y, acc[bb][a][q].x);
                                 acc[bb][a][q].y = fmaf(gr, v[q].y, acc[bb][a][q].y);

@@ -42,7 +42,9 @@ struct grid_plan {
     int traversal, time_block;      // -1 auto / 0 channel-innermost / 1 time-innermost; Tc
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
-    int groups_per_cta, queue_teams;      // variant 3: warp groups per CTA; teams per queue entry (all variants)
+    int groups_per_cta, queue_teams;
+    int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
+    int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on      // variant 3: warp groups per CTA; teams per queue entry (all variants)
     int n_sm, max_smem;
     int last_launches;
     cudaEvent_t ev_start, ev_stop;
@@ -98,32 +100,33 @@ struct WarpDesc {
     size_t (*group_bytes)(int);
 };
 
-template <int CU, int CV, int P, int LOGS, bool OK = (CU <= (1 << LOGS) && CV <= (1 << LOGS))>
+template <int CU, int CV, int P, int LOGS, int PS, bool OK = (CU <= (1 << LOGS) && CV <= (1 << LOGS))>
 struct WarpPick {
     static WarpDesc get() {
-        using T = WarpKernelTraits<CU, CV, P, LOGS>;
-        return WarpDesc{grid_warp_kernel<CU, CV, P, LOGS>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes};
+        using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
+        return WarpDesc{grid_warp_kernel<CU, CV, P, LOGS, PS>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes};
     }
 };
-template <int CU, int CV, int P, int LOGS>
-struct WarpPick<CU, CV, P, LOGS, false> { static WarpDesc get() { return WarpDesc{nullptr, 0, 0, 0, 0, nullptr}; } };
+template <int CU, int CV, int P, int LOGS, int PS>
+struct WarpPick<CU, CV, P, LOGS, PS, false> { static WarpDesc get() { return WarpDesc{nullptr, 0, 0, 0, 0, nullptr}; } };
 
-template <int CU, int CV, int P>
+template <int CU, int CV, int P, int PS>
 WarpDesc pick_warp(int logs) {
     switch (logs) {
-        case 2: return WarpPick<CU, CV, P, 2>::get();
-        case 3: return WarpPick<CU, CV, P, 3>::get();
-        case 4: return WarpPick<CU, CV, P, 4>::get();
-        case 5: return WarpPick<CU, CV, P, 5>::get();
+        case 2: return WarpPick<CU, CV, P, 2, PS>::get();
+        case 3: return WarpPick<CU, CV, P, 3, PS>::get();
+        case 4: return WarpPick<CU, CV, P, 4, PS>::get();
+        case 5: return WarpPick<CU, CV, P, 5, PS>::get();
     }
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
-WarpDesc lookup_warp(int cu, int cv, int P, int logs) {
-#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_warp<a, b, p>(logs);
-    CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
-    CASE(1, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
-    CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
+WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps) {
+#define CASE(a, b, p, s) if (cu == a && cv == b && P == p && ps == s) return pick_warp<a, b, p, s>(logs);
+    CASE(1, 1, 1, 1) CASE(2, 1, 1, 1) CASE(2, 2, 1, 1) CASE(4, 2, 1, 1) CASE(4, 4, 1, 1) CASE(8, 4, 1, 1)
+    CASE(1, 1, 2, 1) CASE(2, 2, 2, 1) CASE(4, 2, 2, 1) CASE(4, 4, 2, 1)
+    CASE(1, 1, 4, 1) CASE(2, 1, 4, 1) CASE(2, 2, 4, 1) CASE(4, 2, 4, 1)
+    CASE(2, 2, 4, 2) CASE(4, 2, 4, 2) CASE(4, 4, 4, 2) CASE(2, 1, 4, 2)
 #undef CASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -134,6 +137,10 @@ int log2_exact(int v) {
 }
 
 size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec); }
+
+// workspace: [256 B counters][order bins][records][chunk order]
+constexpr size_t kHeadBytes = 256 + 2 * kOrderBins * sizeof(uint32_t);
+size_t order_capacity(const grid_plan* p) { return (size_t)(p->n_vis / 16 + 1024); }
 
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
 int derive(grid_plan* p) {
@@ -149,10 +156,10 @@ int derive(grid_plan* p) {
         const int logs = log2_exact(p->S);
         if (logs < 2 || logs > 5)
             return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 32], got %d", p->S);
-        const WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs);
+        const WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
         if (!d.fn)
-            return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols, support %d",
-                        p->cu, p->cv, p->P, p->S);
+            return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
+                        p->cu, p->cv, p->pol_split, p->P, p->S);
         if ((long long)p->W * p->O * 3 * p->S + 2 * p->S > 65535)
             return fail(GRID_ERR_UNSUPPORTED, "variant 3: tap table too large for 16-bit offsets");
         if (p->batch < 4 || (p->batch & (p->batch - 1)) != 0)
@@ -170,7 +177,7 @@ int derive(grid_plan* p) {
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
-        const size_t taps = ((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15;
+        const size_t taps = 16 + (((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15);   // + zero block
         const size_t per_group = d.group_bytes(p->batch);
         if (taps + per_group > (size_t)p->max_smem)
             return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one group's buffers (%zu B) exceed %d B of shared memory",
@@ -258,6 +265,8 @@ void default_tuning(grid_plan* p) {
     p->chunk = 1024;
     p->ctas_per_sm = 2;
     p->traversal = -1;
+    p->sort_chunks = -1;
+    p->pol_split = 1;
     p->time_block = 16;
     // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
     if (p->P >= 4) {
@@ -282,14 +291,35 @@ void default_tuning(grid_plan* p) {
         trial.threads = 1024;              // clipped to the kernel's register-limited maximum
         trial.batch = 32;
         trial.chunk = 256;
-        if (trial.P >= 4) { trial.cu = 2; trial.cv = 2; }
+        // tuned per (S, P) on the BASELINE.json workloads
+        const bool big_grid = (size_t)trial.N * trial.N * trial.P * sizeof(float2) > ((size_t)256 << 20);
+        if (trial.P >= 4) {
+            // grids beyond the L2 are bound by the atomic path: pair lanes so that one grid point
+            // leaves as one 32-byte sector operation (grid_warp_kernel.cuh, PS)
+            if (logs <= 3) { trial.cu = 2; trial.cv = 2; trial.pol_split = big_grid ? 2 : 1; }
+            else if (logs == 4) { trial.cu = 4; trial.cv = 4; trial.pol_split = 2; }
+            else { trial.cu = 4; trial.cv = 2; trial.pol_split = 1; }
+        }
         else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = 2; }
-        else { trial.cu = 4; trial.cv = (logs >= 3) ? 4 : 2; }
+        else if (logs == 2) { trial.cu = 2; trial.cv = 2; }
+        else if (logs == 5) { trial.cu = 8; trial.cv = 4; }
+        else { trial.cu = 4; trial.cv = 4; }
+        // several teams share a warp at small supports: shrink the batch until all warps fit
+        while (trial.batch > 8) {
+            grid_plan probe = trial;
+            if (derive(&probe) != GRID_OK) break;
+            const WarpDesc d = lookup_warp(probe.cu, probe.cv, probe.P, logs, probe.pol_split);
+            if (probe.threads >= d.max_threads - d.gt + 1) break;
+            trial.batch /= 2;
+        }
         if (derive(&trial) == GRID_OK) { *p = trial; return; }
+        trial.pol_split = 1;
     }
     // a bin must fit one CTA
     while (derive(p) != GRID_OK && p->threads < 512) p->threads *= 2;
 }
+
+long long ctas_hint(const grid_plan* p) { return (long long)p->n_sm * (p->groups_per_cta > 0 ? p->groups_per_cta : 1); }
 
 QuantParams quant_params(const grid_plan* p) {
     QuantParams q;
@@ -360,7 +390,7 @@ int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_ch
 
 size_t grid_plan_workspace_bytes(const grid_plan* plan) {
     if (!plan || plan->n_vis < 0) return 0;
-    return 256 + records_bytes(plan);
+    return kHeadBytes + records_bytes(plan) + order_capacity(plan) * sizeof(uint32_t);
 }
 
 int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
@@ -384,7 +414,11 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     if (ctas_per_sm > 0) trial.ctas_per_sm = ctas_per_sm;
     if (trial.variant < 0 || trial.variant > 3)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: unknown variant %d", trial.variant);
-    const int rc = derive(&trial);
+    int rc = derive(&trial);
+    if (rc != GRID_OK && trial.pol_split != 1 && (cu > 0 || cv > 0 || variant >= 0)) {
+        trial.pol_split = 1;                // a block the current polarisation split does not offer
+        rc = derive(&trial);
+    }
     if (rc != GRID_OK) return rc;
     *plan = trial;
     return GRID_OK;
@@ -392,9 +426,10 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
 
 int grid_plan_get_info(const grid_plan* plan, int* out) {
     if (!plan || !out) return fail(GRID_ERR_INVALID_ARG, "grid_plan_get_info: null argument");
-    const int v[16] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
+    const int v[20] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
                        plan->teams_per_cta, plan->threads, plan->batch, plan->chunk, plan->ctas_per_sm,
-                       plan->smem_bytes, plan->n_sm, plan->traversal, plan->time_block, 0};
+                       plan->smem_bytes, plan->n_sm, plan->traversal, plan->time_block, plan->sort_chunks,
+                       plan->pol_split, plan->groups_per_cta, 0, 0};
     memcpy(out, v, sizeof(v));
     return GRID_OK;
 }
@@ -404,6 +439,25 @@ int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block) {
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_traversal: mode in {-1,0,1}, time_block a power of two or 0");
     plan->traversal = mode;
     if (time_block > 0) plan->time_block = time_block;
+    return GRID_OK;
+}
+
+int grid_plan_set_pol_split(grid_plan* plan, int lanes) {
+    if (!plan || (lanes != 1 && lanes != 2))
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_pol_split: lanes in {1,2}");
+    grid_plan trial = *plan;
+    trial.pol_split = lanes;
+    trial.threads = 1024;
+    const int rc = derive(&trial);
+    if (rc != GRID_OK) return rc;
+    *plan = trial;
+    return GRID_OK;
+}
+
+int grid_plan_set_chunk_order(grid_plan* plan, int mode) {
+    if (!plan || mode < -1 || mode > 1)
+        return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_chunk_order: mode in {-1,0,1}");
+    plan->sort_chunks = mode;
     return GRID_OK;
 }
 
@@ -443,7 +497,9 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         return fail(GRID_ERR_STATE, "grid_execute: workspace missing or smaller than grid_plan_workspace_bytes()");
 
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
-    SampleRec* recs = reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + 256);
+    SampleRec* recs = reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
+    uint32_t* bins = counters + 64;
+    uint32_t* order = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(recs) + records_bytes(plan));
 
     // the layout hint is used only if it is consistent with the sample count
     const bool have_layout = plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
@@ -452,7 +508,7 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     float* hop_stats = reinterpret_cast<float*>(counters + 2);
 
     // reset the chunk queue and the hop statistics, then a1: quantise pass
-    if (cudaMemsetAsync(counters, 0, 256, stream) != cudaSuccess)
+    if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
     {
         const long long threads = (plan->n_vis + 3) / 4;
@@ -477,8 +533,8 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     gp.team_threads = plan->team_threads; gp.teams_per_cta = plan->teams_per_cta;
     gp.batch = plan->batch; gp.chunk = plan->chunk;
 
-    if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
     if (plan->variant == 0) {
+        if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
         const long long total = plan->n_vis * plan->S;
         const long long blocks = (total + 255) / 256;
         if (blocks > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_execute: too many samples for the scatter variant");
@@ -533,11 +589,30 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);
-        kernel_fn fn = plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs).fn
+        kernel_fn fn = plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
                      : plan->variant == 2 ? lookup_cyclic(plan->cu, plan->cv, plan->P, logs)
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
+        // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
+        if (plan->variant == 3) {
+            const long long chunks_a = (plan->n_vis + gp.chunk - 1) / gp.chunk;
+            const long long max_chunks = chunks_a > gp.n_chunks_b ? chunks_a : gp.n_chunks_b;
+            const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
+            const bool want = plan->sort_chunks > 0 || (plan->sort_chunks < 0 && grid_bytes > ((size_t)256 << 20));
+            if (want && max_chunks <= (long long)order_capacity(plan) && max_chunks >= 4LL * ctas_hint(plan)) {
+                int ts = 0;
+                while ((plan->N >> ts) > 32) ++ts;
+                gp.tile_shift = ts;
+                const unsigned blocks = (unsigned)((max_chunks + 255) / 256);
+                chunk_histogram_kernel<<<blocks, 256, 0, stream>>>(gp, bins);
+                chunk_scan_kernel<<<1, kOrderBins, 0, stream>>>(bins);
+                chunk_scatter_kernel<<<blocks, 256, 0, stream>>>(gp, bins, order);
+                gp.order = order;
+                plan->last_launches += 3;
+            }
+        }
         cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, plan->smem_bytes);
         if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
         long long ctas = (long long)plan->n_sm * plan->ctas_per_sm;
         const long long need = (max_groups + queues - 1) / queues;
         if (ctas > need) ctas = need;

@@ -48,6 +48,8 @@ struct GridParams {
     // layout hint (0 = unknown) and time-innermost traversal: a mode-1 chunk is tc time steps x all
     // channels of one baseline; a batch is tc x (1 << cb_shift) samples
     int n_chan, n_times, tc, cb_shift, n_tblocks;
+    const uint32_t* order;    // variant 3: queue position -> chunk id (chunk_order.cuh); null = identity
+    int tile_shift;           // log2 of the tile side used for that order
     int n_cblocks, chunk_cols;   // variant 3, time-innermost: a chunk spans chunk_cols channels
     int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
 };

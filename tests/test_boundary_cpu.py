@@ -45,7 +45,7 @@ def test_plan_validation(binding):
 def test_default_plan_geometry(binding, S, P):
     plan = binding.GridPlan(4096, S, 8, 16, P)
     i = plan.info()
-    if i["variant"] == 2:
+    if i["variant"] in (2, 3):
         # power-of-two support: bin == support, owned positions S/C apart (north_star: "taken modulo the support")
         assert S in (4, 8, 16, 32) and i["bin_u"] == i["bin_v"] == S
     else:
@@ -53,9 +53,9 @@ def test_default_plan_geometry(binding, S, P):
         assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
         assert S + i["cu"] - 1 <= i["bin_u"] < S + 2 * i["cu"] - 1
         assert S + i["cv"] - 1 <= i["bin_v"] < S + 2 * i["cv"] - 1
-    assert i["team_threads"] == (i["bin_u"] // i["cu"]) * (i["bin_v"] // i["cv"])
+    assert i["team_threads"] == (i["bin_u"] // i["cu"]) * (i["bin_v"] // i["cv"]) * max(i["pol_split"], 1)
     assert 1 <= i["teams_per_cta"] <= i["threads_per_cta"] // i["team_threads"]
-    assert i["cu"] * i["cv"] * P <= 32
+    assert i["cu"] * i["cv"] * P // max(i["pol_split"], 1) <= 32
     assert i["smem_bytes"] <= 227 * 1024
     plan.destroy()
 
@@ -64,9 +64,10 @@ def test_workspace_and_tuning(binding):
     plan = binding.GridPlan(2048, 8, 8, 1, 4)
     assert plan.workspace_bytes() == 0              # set_samples not called yet
     plan.set_samples(1001)
-    assert plan.workspace_bytes() == 256 + 1004 * 16
+    head = 256 + 2 * 1024 * 4                       # counters + chunk-order bins
+    assert plan.workspace_bytes() == head + 1004 * 16 + (1001 // 16 + 1024) * 4
     plan.set_samples(0)
-    assert plan.workspace_bytes() == 256
+    assert plan.workspace_bytes() == head + 1024 * 4
     plan.set_layout(10, 10, 10)
     plan.set_tuning(variant=1, cu=2, cv=2, threads_per_cta=128, batch=32, chunk=512, ctas_per_sm=3)
     i = plan.info()

@@ -141,6 +141,24 @@ def test_every_warp_block(oracle_mod, cu, cv, P, S):
         assert_parity(got, ref, f"warp C={cu}x{cv} P={P} S={S} batch={batch} {info}")
 
 
+@pytest.mark.parametrize("cu,cv", [(2, 1), (2, 2), (4, 2), (4, 4)])
+@pytest.mark.parametrize("S", [4, 8, 16, 32])
+def test_warp_block_pol_split(oracle_mod, cu, cv, S):
+    # 4 polarisations spread over lane pairs (grid_plan_set_pol_split): same result as the oracle
+    if cu > S or cv > S:
+        pytest.skip("block larger than the support")
+    N, O, W, P, n = 128, 4, 3, 4, 20_003
+    uvw, vis, wts, kernel = synth.random_problem(3000 + 10 * cu + cv + S, n, N, S, O, W, P, spread=0.5, walk=1.5)
+    uvw[5000:5100, :2] = np.random.default_rng(S).uniform(-60, 60, (100, 2))
+    uvw[7000:7010, 0] = np.nan
+    vis[7000:7010] = np.inf
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                        tuning=dict(pol_split=2, variant=3, cu=cu, cv=cv, threads_per_cta=1024, batch=16, chunk=200))
+    assert (info["variant"], info["cu"], info["cv"]) == (3, cu, cv)
+    assert_parity(got, ref, f"pol-split C={cu}x{cv} S={S} {info}")
+
+
 @pytest.mark.parametrize("S,P,cu,cv", [(1, 1, 1, 1), (2, 4, 2, 1), (3, 1, 2, 2), (4, 1, 4, 2), (5, 2, 2, 2),
                                        (16, 1, 4, 4), (16, 4, 2, 2), (32, 1, 8, 4), (32, 4, 4, 2), (13, 1, 4, 4)])
 def test_supports(oracle_mod, S, P, cu, cv):

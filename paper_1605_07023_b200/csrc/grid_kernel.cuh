@@ -13,18 +13,10 @@
 namespace gridb200 {
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
-#ifdef GRIDB200_PROBE_NO_RED      /* measurement probe only: keeps the operands live, issues nothing */
-    asm volatile("" :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
-    return;
-#endif
     asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
                  :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 __device__ __forceinline__ void red_add_v2(float* addr, float a, float b) {
-#ifdef GRIDB200_PROBE_NO_RED
-    asm volatile("" :: "l"(addr), "f"(a), "f"(b) : "memory");
-    return;
-#endif
     asm volatile("red.relaxed.gpu.global.add.v2.f32 [%0], {%1, %2};"
                  :: "l"(addr), "f"(a), "f"(b) : "memory");
 }

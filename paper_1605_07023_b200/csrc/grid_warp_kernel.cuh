@@ -80,7 +80,7 @@ grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
     constexpr int PT = T::PT;
     constexpr int S = T::S, DU = T::DU, DV = T::DV, TEAM = T::TEAM, GW = T::GW, GT = T::GT, TPG = T::TPG;
-    constexpr int ROW = 3 * S;                         // tripled tap row: k[t mod S], t < 3S
+    constexpr int ROW = 2 * S;                         // doubled tap row k[t mod S], t < 2S: offsets reach 2S-1
     constexpr bool WIDE = S > 16;                      // record format: 32-bit masks need two words
     static_assert(CU <= S && CV <= S, "block larger than the support");
 
@@ -391,9 +391,6 @@ grid_warp_kernel(const GridParams gp) {
                 bool moved;
                 if constexpr (WIDE) moved = ((c.z & MX) | (c.w & MY)) != 0;
                 else moved = (c.w & MXY) != 0;
-#ifdef GRIDB200_PROBE_NO_FLUSH                             /* measurement probe only (wrong results) */
-                moved = false;
-#endif
                 if (moved) {                           // a5/a8: some of my points moved
                     const int i0 = (int)(c.x & 0x7fffu), j0 = (int)(c.x >> 16);
                     const uint32_t mxs = (WIDE ? c.z : c.w) >> r0;
@@ -442,9 +439,6 @@ grid_warp_kernel(const GridParams gp) {
                     v[0] = *vp;
                 }
                 vp += P;
-#ifdef GRIDB200_PROBE_NO_MAC                               /* measurement probe only (wrong results) */
-                if (gu[0].x == 12345.678f)
-#endif
                 if constexpr (PT < CU) {
                     // a6 reordered: T = Gv_j * V_p first, then Gu_i * T
 #pragma unroll

@@ -140,7 +140,7 @@ size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 
 
 // workspace: [256 B counters][order bins][records][chunk order]
 constexpr size_t kHeadBytes = 256 + 2 * kOrderBins * sizeof(uint32_t);
-size_t order_capacity(const grid_plan* p) { return (size_t)(p->n_vis / 16 + 1024); }
+size_t order_capacity(const grid_plan* p) { return (size_t)(p->n_vis / 8 + 4096); }
 
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
 int derive(grid_plan* p) {
@@ -160,7 +160,7 @@ int derive(grid_plan* p) {
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
                         p->cu, p->cv, p->pol_split, p->P, p->S);
-        if ((long long)p->W * p->O * 3 * p->S + 2 * p->S > 65535)
+        if ((long long)p->W * p->O * 2 * p->S > 65535)
             return fail(GRID_ERR_UNSUPPORTED, "variant 3: tap table too large for 16-bit offsets");
         if (p->batch < 4 || (p->batch & (p->batch - 1)) != 0)
             return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two >= 4", p->batch);
@@ -171,13 +171,13 @@ int derive(grid_plan* p) {
         if (threads < d.gt)
             return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA may have %d", d.gt, threads);
         p->bin_u = p->bin_v = p->S;
-        p->row_u = p->row_v = 3 * p->S;
+        p->row_u = p->row_v = 2 * p->S;
         p->nbx = p->S / p->cu;
         p->nby = p->S / p->cv;
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
-        const size_t taps = 16 + (((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15);   // + zero block
+        const size_t taps = 16 + (((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15);   // + zero block
         const size_t per_group = d.group_bytes(p->batch);
         if (taps + per_group > (size_t)p->max_smem)
             return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one group's buffers (%zu B) exceed %d B of shared memory",
@@ -598,7 +598,8 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
             const long long max_chunks = chunks_a > gp.n_chunks_b ? chunks_a : gp.n_chunks_b;
             const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
             const bool want = plan->sort_chunks > 0 || (plan->sort_chunks < 0 && grid_bytes > ((size_t)256 << 20));
-            if (want && max_chunks <= (long long)order_capacity(plan) && max_chunks >= 4LL * ctas_hint(plan)) {
+            const bool worth = plan->sort_chunks > 0 || max_chunks >= 4LL * ctas_hint(plan);   // auto: only when chunks queue up
+            if (want && worth && max_chunks <= (long long)order_capacity(plan)) {
                 int ts = 0;
                 while ((plan->N >> ts) > 32) ++ts;
                 gp.tile_shift = ts;

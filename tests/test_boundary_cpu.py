@@ -65,9 +65,9 @@ def test_workspace_and_tuning(binding):
     assert plan.workspace_bytes() == 0              # set_samples not called yet
     plan.set_samples(1001)
     head = 256 + 2 * 1024 * 4                       # counters + chunk-order bins
-    assert plan.workspace_bytes() == head + 1004 * 16 + (1001 // 16 + 1024) * 4
+    assert plan.workspace_bytes() == head + 1004 * 16 + (1001 // 8 + 4096) * 4
     plan.set_samples(0)
-    assert plan.workspace_bytes() == head + 1024 * 4
+    assert plan.workspace_bytes() == head + 4096 * 4
     plan.set_layout(10, 10, 10)
     plan.set_tuning(variant=1, cu=2, cv=2, threads_per_cta=128, batch=32, chunk=512, ctas_per_sm=3)
     i = plan.info()

@@ -202,6 +202,24 @@ def test_traversal_modes(oracle_mod, mode, n_ant, n_times, n_chan, tc):
         assert_parity(got, ref, f"{name} mode={mode}")
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("name,ps", [("cfg1", 1), ("cfg3", 2), ("cfg2", 1)])
+def test_sorted_chunk_queue(oracle_mod, name, ps, mode):
+    # chunk ids sorted by grid tile (grid_plan_set_chunk_order): same sum, both traversal modes, small chunks
+    cfg = synth.shrink(synth.get_config(name), n_ant=14, n_times=40, n_chan=24, grid_size=1024)
+    wl = synth.make_workload(cfg)
+    ref = oracle_mod.grid(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                          wl.uvw, wl.vis, wl.weights, wl.kernel)
+    tuning = dict(chunk_order=1, traversal=mode, chunk=64, batch=16)
+    if cfg.n_pol == 4:
+        tuning["pol_split"] = ps
+    got, info = run_gpu(cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol,
+                        wl.uvw, wl.vis, wl.weights, wl.kernel,
+                        layout=(cfg.n_baselines, cfg.n_times, cfg.n_chan), tuning=tuning)
+    assert info["chunk_order"] == 1 and info["launches"] == 5
+    assert_parity(got, ref, f"{name} sorted queue mode={mode}")
+
+
 def test_inconsistent_layout_hint_is_ignored(oracle_mod):
     cfg = synth.shrink(synth.get_config("cfg1"), n_ant=8, n_times=16, n_chan=8, grid_size=256)
     wl = synth.make_workload(cfg)

@@ -227,8 +227,7 @@ def run_ours(args):
         plan.set_tuning(**tuning)
     plan.allocate_workspace(dev)
     info = plan.info()
-    kernel_name = {0: "grid_scatter_kernel", 1: "grid_coarsened_kernel", 2: "grid_cyclic_kernel",
-                   3: "grid_warp_kernel"}[info["variant"]]
+    kernel_name = {0: "grid_scatter_kernel", 1: "grid_coarsened_kernel", 3: "grid_warp_kernel"}[info["variant"]]
     kernel_name += "<%d,%d,%d>" % (info["cu"], info["cv"], P)
 
     # number of valid samples (for the metric) from the library's own quantise pass

@@ -4,10 +4,12 @@
 // fixed position modulo the bin and keeps the one inside the current footprint in a register
 // accumulator, flushing it with an atomic add when it changes.  Thread coarsening:
 // each thread owns Cu x Cv positions, so tap loads, the "did my points move" test and the loop
-// overhead are paid once per block of Cu*Cv*P accumulators.  As in grid_cyclic_kernel.cuh the bin
-// equals the support (no zero padding) and the Cu (Cv) positions of a thread are S/Cu (S/Cv) apart.
+// overhead are paid once per block of Cu*Cv*P accumulators.  The bin equals the support (no zero
+// padding: the paper's aligned, padded box wastes 36-56 % of the FMAs at S = 8-16, its own caveat for
+// small GCFs) and the Cu (Cv) positions of a thread are S/Cu (S/Cv) apart, so every
+// owned position is an independent Romein column/row and never wraps.
 //
-// What is new relative to the paper's kernel and to variant 2, and why (B200 measurements in
+// What is new relative to the paper's kernel, and why (B200 measurements in
 // DESIGN.md section 6):
 //   * on sm_100a integer/logic instructions cost 1.5-2 issue cycles against 1 for an FFMA, so the
 //     flush path decides the rate once samples hop by a cell or more (BASELINE.json's data: 0.6
@@ -23,10 +25,27 @@
 //     next batch is in flight.
 #pragma once
 #include "gridder_common.cuh"
-#include "grid_cyclic_kernel.cuh"      // moved_mask<>, flush helpers
+#include "grid_kernel.cuh"             // red_add_v2 / red_add_v4
 #include "chunk_order.cuh"
 
 namespace gridb200 {
+
+// Bit mask of the bin positions whose grid point changes when the footprint origin goes from
+// `from` to `to` (one axis).  All positions if it jumps by a whole support or more.
+template <int LOGS>
+__device__ __forceinline__ uint32_t moved_mask(int from, int to) {
+    constexpr int S = 1 << LOGS;
+    constexpr uint32_t ALL = 0xffffffffu >> (32 - S);
+    const int d = to - from;
+    if (d == 0) return 0u;
+    const int ad = d < 0 ? -d : d;
+    if (ad >= S) return ALL;
+    const int start = (d > 0 ? from : to) & (S - 1);        // positions start .. start+ad-1 (cyclic)
+    const uint32_t run = (1u << ad) - 1u;
+    uint32_t m = run << start;
+    if constexpr (S < 32) m |= m >> S; else m |= (start ? run >> (32 - start) : 0u);
+    return m & ALL;
+}
 
 struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
     long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)

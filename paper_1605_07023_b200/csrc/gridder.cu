@@ -7,7 +7,6 @@
 #include <cstring>
 #include <new>
 
-#include "grid_cyclic_kernel.cuh"
 #include "grid_kernel.cuh"
 #include "grid_warp_kernel.cuh"
 #include "gridder_common.cuh"
@@ -63,32 +62,6 @@ kernel_fn lookup_kernel(int cu, int cv, int P) {
     CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 1, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 2, 1) CASE(8, 4, 1)
     CASE(1, 1, 2) CASE(2, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
     CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 1, 4) CASE(4, 2, 4)
-#undef CASE
-    return nullptr;
-}
-
-template <int CU, int CV, int P, int LOGS, bool OK = (CU <= (1 << LOGS) && CV <= (1 << LOGS))>
-struct CycPick { static kernel_fn get() { return grid_cyclic_kernel<CU, CV, P, LOGS>; } };
-template <int CU, int CV, int P, int LOGS>
-struct CycPick<CU, CV, P, LOGS, false> { static kernel_fn get() { return nullptr; } };
-
-template <int CU, int CV, int P>
-kernel_fn pick_cyc(int logs) {
-    switch (logs) {
-        case 2: return CycPick<CU, CV, P, 2>::get();
-        case 3: return CycPick<CU, CV, P, 3>::get();
-        case 4: return CycPick<CU, CV, P, 4>::get();
-        case 5: return CycPick<CU, CV, P, 5>::get();
-    }
-    return nullptr;
-}
-
-// Power-of-two supports 4..32 (bin == support, no padding).
-kernel_fn lookup_cyclic(int cu, int cv, int P, int logs) {
-#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_cyc<a, b, p>(logs);
-    CASE(1, 1, 1) CASE(2, 1, 1) CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
-    CASE(1, 1, 2) CASE(2, 2, 2) CASE(4, 2, 2)
-    CASE(1, 1, 4) CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
 #undef CASE
     return nullptr;
 }
@@ -192,38 +165,6 @@ int derive(grid_plan* p) {
         p->smem_bytes = (int)(taps + (size_t)groups * per_group);
         return GRID_OK;
     }
-    if (p->variant == 2) {
-        const int logs = log2_exact(p->S);
-        if (logs < 2 || logs > 5)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 2 needs a power-of-two support in [4, 32], got %d", p->S);
-        if (!lookup_cyclic(p->cu, p->cv, p->P, logs))
-            return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols, support %d",
-                        p->cu, p->cv, p->P, p->S);
-        if ((long long)p->W * p->O * 3 * p->S + 2 * p->S > 65535)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 2: tap table too large for 16-bit offsets");
-        p->bin_u = p->bin_v = p->S;
-        p->row_u = p->row_v = 3 * p->S;
-        p->nbx = p->S / p->cu;
-        p->nby = p->S / p->cv;
-        p->team_threads = p->nbx * p->nby;
-        if (p->threads % 32 != 0 || p->threads < 32 || p->threads > 512)
-            return fail(GRID_ERR_UNSUPPORTED, "threads_per_cta %d must be a multiple of 32 in [32, 512]", p->threads);
-        if (p->team_threads > p->threads)
-            return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA has %d", p->team_threads, p->threads);
-        if (p->batch < 1 || (p->batch & (p->batch - 1)) != 0)
-            return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two", p->batch);
-        if (p->chunk < 1) return fail(GRID_ERR_UNSUPPORTED, "chunk %d must be positive", p->chunk);
-        p->teams_per_cta = p->threads / p->team_threads;
-        size_t taps = ((size_t)p->W * p->O * 3 * p->S * sizeof(float2) + 15) & ~(size_t)15;
-        const size_t per_team = (size_t)p->batch * (sizeof(uint4) + (size_t)p->P * sizeof(float2));
-        if (taps + per_team > (size_t)p->max_smem)
-            return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one batch buffer (%zu B) exceed %d B of shared memory",
-                        taps, per_team, p->max_smem);
-        const size_t fit = ((size_t)p->max_smem - taps) / per_team;
-        if ((size_t)p->teams_per_cta > fit) p->teams_per_cta = (int)fit;
-        p->smem_bytes = (int)(taps + (size_t)p->teams_per_cta * per_team);
-        return GRID_OK;
-    }
     if (!lookup_kernel(p->cu, p->cv, p->P))
         return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d is not instantiated for %d pols", p->cu, p->cv, p->P);
     // bin >= S + C - 1, multiple of the block
@@ -283,7 +224,7 @@ void default_tuning(grid_plan* p) {
         else { p->cu = 2; p->cv = 2; }
     }
     if (p->S < 4) { p->cu = 1; p->cv = 1; }
-    // power-of-two supports: bin == support, no padding (grid_cyclic_kernel.cuh)
+    // power-of-two supports: bin == support, no padding (grid_warp_kernel.cuh)
     const int logs = log2_exact(p->S);
     if (logs >= 2 && logs <= 5) {
         grid_plan trial = *p;
@@ -323,7 +264,7 @@ long long ctas_hint(const grid_plan* p) { return (long long)p->n_sm * (p->groups
 
 QuantParams quant_params(const grid_plan* p) {
     QuantParams q;
-    q.format = p->variant >= 2 ? 1 : 0;
+    q.format = p->variant == 3 ? 1 : 0;
     q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
     q.oversample = p->O;
     q.shift = p->O - (p->O * p->S + 1) / 2;
@@ -412,7 +353,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     if (batch > 0) trial.batch = batch;
     if (chunk > 0) trial.chunk = chunk;
     if (ctas_per_sm > 0) trial.ctas_per_sm = ctas_per_sm;
-    if (trial.variant < 0 || trial.variant > 3)
+    if (trial.variant < 0 || trial.variant > 3 || trial.variant == 2)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: unknown variant %d", trial.variant);
     int rc = derive(&trial);
     if (rc != GRID_OK && trial.pol_split != 1 && (cu > 0 || cv > 0 || variant >= 0)) {
@@ -590,7 +531,6 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);
         kernel_fn fn = plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
-                     : plan->variant == 2 ? lookup_cyclic(plan->cu, plan->cv, plan->P, logs)
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
         if (plan->variant == 3) {

@@ -16,7 +16,7 @@ namespace gridb200 {
 typedef uint4 SampleRec;
 static constexpr uint32_t kInvalidRec = 0xFFFFFFFFu;
 
-// Record of the power-of-two-support kernel (grid_cyclic_kernel.cuh), 8 bytes:
+// Record of the power-of-two-support kernel (grid_warp_kernel.cuh), 8 bytes:
 //   pos : i0 | skipped << 15 | j0 << 16   (a skipped sample carries clamped in-grid coordinates)
 //   rows: (wp*O + su) | (wp*O + sv) << 16
 struct CycRec { uint32_t pos, rows; };

@@ -14,7 +14,7 @@ __device__ __forceinline__ bool quantise_axis(float x, const QuantParams& qp, in
     const double pos = floor(fma((double)x, (double)qp.oversample, qp.c_centre));
     const double q = pos + (double)qp.shift;
     const bool ok = (q >= 0.0 && q < (double)qp.q_limit);        // false for NaN, Inf, outside the grid
-    // skipped samples still get in-grid coordinates (fmax/fmin drop NaN): the cyclic kernel walks them
+    // skipped samples still get in-grid coordinates (fmax/fmin drop NaN): the bin == support kernel walks them
     const int qi = (int)fmin(fmax(q, 0.0), (double)(qp.q_limit - 1));
     const int c = qi / qp.oversample;
     *cell = c;

@@ -45,7 +45,7 @@ def test_plan_validation(binding):
 def test_default_plan_geometry(binding, S, P):
     plan = binding.GridPlan(4096, S, 8, 16, P)
     i = plan.info()
-    if i["variant"] in (2, 3):
+    if i["variant"] == 3:
         # power-of-two support: bin == support, owned positions S/C apart (north_star: "taken modulo the support")
         assert S in (4, 8, 16, 32) and i["bin_u"] == i["bin_v"] == S
     else:

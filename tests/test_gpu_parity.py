@@ -90,32 +90,6 @@ def test_every_coarsening_block(oracle_mod, cu, cv, P, S):
     assert_parity(got, ref, f"C={cu}x{cv} P={P} S={S}")
 
 
-CYCLIC = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (1, 1, 2), (2, 2, 2), (4, 2, 2),
-          (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 2, 4)]
-
-
-@pytest.mark.parametrize("cu,cv,P", CYCLIC)
-@pytest.mark.parametrize("S", [4, 8, 16, 32])
-def test_every_cyclic_block(oracle_mod, cu, cv, P, S):
-    # bin == support kernel (variant 2): ragged tail, samples off the grid (walked with zero
-    # visibilities), jumps larger than the support, three planes
-    team = (S // max(cu, 1)) * (S // max(cv, 1))
-    if cu > S or cv > S or team > 512:
-        pytest.skip("block larger than the support, or bin larger than a CTA")
-    threads = max(128, (team + 31) // 32 * 32)
-    N, O, W, n = 128, 4, 3, 20_003
-    uvw, vis, wts, kernel = synth.random_problem(1000 + 100 * cu + 10 * cv + P + S, n, N, S, O, W, P,
-                                                 spread=0.5, walk=1.5)
-    uvw[5000:5100, :2] = np.random.default_rng(S).uniform(-60, 60, (100, 2))    # big jumps
-    uvw[7000:7010, 0] = np.nan
-    vis[7000:7010] = np.inf
-    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
-    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
-                        tuning=dict(variant=2, cu=cu, cv=cv, threads_per_cta=threads, batch=32, chunk=300))
-    assert (info["variant"], info["cu"], info["cv"], info["bin_u"]) == (2, cu, cv, S)
-    assert_parity(got, ref, f"cyclic C={cu}x{cv} P={P} S={S}")
-
-
 WARP = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (1, 1, 2), (2, 2, 2), (4, 2, 2), (4, 4, 2),
         (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 2, 4)]
 

@@ -224,7 +224,7 @@ grid_warp_kernel(const GridParams gp) {
 
     const int mode = pick_mode(gp);
     const long long n_groups = mode ? gp.n_groups_b : gp.n_groups_a;
-    const int n_batches = mode ? (gp.chunk_cols + (1 << gp.cb_shift) - 1) >> gp.cb_shift
+    const int n_batches = mode ? (gp.chunk_cols * gp.tc + B - 1) >> bshift
                                : (gp.chunk + B - 1) >> bshift;
 
     // a9: take the next chunk group from the queue; lanes t < TPG work out their team's geometry
@@ -280,9 +280,8 @@ grid_warp_kernel(const GridParams gp) {
             const int left = cg.len - (b << bshift);
             return left < 0 ? 0 : (left < B ? left : B);
         }
-        int cols = cg.len - (b << gp.cb_shift);
-        if (cols > (1 << gp.cb_shift)) cols = 1 << gp.cb_shift;
-        return cols < 0 ? 0 : cols * cg.h;
+        const int left = cg.len * cg.h - (b << bshift);        // columns of h time steps, walked one after another
+        return left < 0 ? 0 : (left < B ? left : B);
     };
 
     auto sample_of = [&](const WarpChunk& cg, int b, int k) -> long long {
@@ -297,8 +296,9 @@ grid_warp_kernel(const GridParams gp) {
             }
             return a;
         }
-        const int ci = (int)((uint32_t)k / (uint32_t)cg.h), tt = k - ci * cg.h;
-        const int col = cg.col0 + (b << gp.cb_shift) + ci;
+        const int q = (b << bshift) + k;
+        const int ci = (int)((uint32_t)q / (uint32_t)cg.h), tt = q - ci * cg.h;
+        const int col = cg.col0 + ci;
         const int ti = (col & 1) ? cg.h - 1 - tt : tt;
         return cg.base + (long long)ti * gp.n_chan + col;
     };

@@ -208,7 +208,7 @@ void default_tuning(grid_plan* p) {
     p->traversal = -1;
     p->sort_chunks = -1;
     p->pol_split = 1;
-    p->time_block = 16;
+    p->time_block = 64;
     // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
     if (p->P >= 4) {
         if (p->S >= 24) { p->cu = 4; p->cv = 2; }
@@ -505,21 +505,28 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         gp.hop_stats = hop_stats;
         gp.force_mode = have_layout ? plan->traversal : 0;
         gp.n_chan = n_chan; gp.n_times = n_times;
-        int tc = plan->time_block < plan->batch ? plan->time_block : plan->batch;
+        // the padded kernel stages whole columns per batch (tc <= batch); the warp kernel does not care
+        int tc = plan->time_block;
+        if (plan->variant != 3) {
+            if (tc > plan->batch) tc = plan->batch;
+            if (tc > 16) tc = 16;          // its chunks are whole (baseline, time block) slabs: keep them small
+            // small inputs: shorter time blocks until every team has a chunk
+            while (have_layout && tc > 4 &&
+                   (long long)plan->n_baselines * ((n_times + tc - 1) / tc) < want_groups * qt / 4) tc /= 2;
+        }
         if (have_layout) {
             while (tc > 1 && tc / 2 >= n_times) tc /= 2;
             int tshift = 0;
             while ((1 << tshift) < tc) ++tshift;
             gp.tc = tc;
-            gp.cb_shift = shift - tshift;
+            gp.cb_shift = shift > tshift ? shift - tshift : 0;
             gp.n_tblocks = (n_times + tc - 1) / tc;
             gp.n_cblocks = 1;
             gp.chunk_cols = n_chan;
             if (plan->variant == 3) {      // chunk = tc time steps x chunk_cols channels ~ gp.chunk samples
-                const int cpb = 1 << gp.cb_shift;
-                int cols = (gp.chunk / tc + cpb - 1) / cpb * cpb;
-                if (cols < cpb) cols = cpb;
-                if (cols > n_chan) cols = (n_chan + cpb - 1) / cpb * cpb;
+                int cols = gp.chunk / tc;
+                if (cols < 1) cols = 1;
+                if (cols > n_chan) cols = n_chan;
                 gp.chunk_cols = cols;
                 gp.n_cblocks = (n_chan + cols - 1) / cols;
             }

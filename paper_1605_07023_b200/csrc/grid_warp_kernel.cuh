@@ -104,11 +104,8 @@ grid_warp_kernel(const GridParams gp) {
     static_assert(CU <= S && CV <= S, "block larger than the support");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // [0, 16): zeros.  Accumulators are cleared with one LDS.128 from here instead of four moves: the
-    // moves ptxas emits (IMAD.U32 Rx, RZ, RZ, URy) occupy the FMA pipe the kernel is short of.
-    const uint32_t zero_addr = (uint32_t)__cvta_generic_to_shared(smem_raw);
-    float2* taps = reinterpret_cast<float2*>(smem_raw + 16);
-    const size_t taps_bytes = 16 + (((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15);
+    float2* taps = reinterpret_cast<float2*>(smem_raw);
+    const size_t taps_bytes = ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
     const int B = gp.batch, bshift = gp.batch_shift;
     const int slots = TPG * B;
 
@@ -124,7 +121,6 @@ grid_warp_kernel(const GridParams gp) {
     uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
     uint32_t* ctrl = last_pos + 2 * TPG;
 
-    if (tid < 4) reinterpret_cast<float*>(smem_raw)[tid] = 0.f;
     for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {          // a4
         const int r = k / ROW, t = (k - r * ROW) & (S - 1);
         taps[k] = __ldg(gp.kern + (size_t)r * S + t);
@@ -173,17 +169,11 @@ grid_warp_kernel(const GridParams gp) {
     float* gridp = gp.grid;
     asm volatile("" : "+l"(gridp));
 
+    // (clearing by a reload of zeros from shared memory was tried: ptxas still copies the loaded
+    //  registers into the accumulators one by one, so plain assignments are kept)
     auto clear_point = [&](float2 (&v)[PT]) {
-        if constexpr (PT == 4) {
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%8];\n\tld.shared.v4.f32 {%4, %5, %6, %7}, [%8];"
-                         : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y),
-                           "=f"(v[3].x), "=f"(v[3].y) : "r"(zero_addr));
-        } else if constexpr (PT == 2) {
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                         : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y) : "r"(zero_addr));
-        } else {
-            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v[0].x), "=f"(v[0].y) : "r"(zero_addr));
-        }
+#pragma unroll
+        for (int q = 0; q < PT; ++q) v[q] = make_float2(0.f, 0.f);
     };
 
     // a8: one grid point, all polarisations: atomic add, then clear

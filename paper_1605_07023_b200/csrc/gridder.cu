@@ -150,7 +150,7 @@ int derive(grid_plan* p) {
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
-        const size_t taps = 16 + (((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15);   // + zero block
+        const size_t taps = ((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15;
         const size_t per_group = d.group_bytes(p->batch);
         if (taps + per_group > (size_t)p->max_smem)
             return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one group's buffers (%zu B) exceed %d B of shared memory",

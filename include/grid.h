@@ -97,7 +97,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
  * sum in a different order, pin P11): mode -1 = choose per call from the mean hop between
  * consecutive samples measured by the quantise pass (default), 0 = input order (channel innermost,
  * odd time rows mirrored), 1 = time innermost over blocks of `time_block` time steps (power of two,
- * <= batch; 0 keeps the current value).  PAPER.md:61, 107: the gain of register accumulation depends
+ * default 64; the padded kernel caps it at min(batch, 16); 0 keeps the current value).  PAPER.md:61, 107: the gain of register accumulation depends
  * on "the coordinates and ordering of the data". */
 int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block);
 

@@ -20,7 +20,7 @@ __device__ __forceinline__ int pick_mode(const GridParams& gp) {
     int mode = gp.force_mode;
     if (mode < 0) {
         mode = 0;
-        if (gp.n_chan > 0) {
+        if (gp.n_chan > 1) {                    // one channel: input order already is time-innermost
             const float hc = __ldg(gp.hop_stats), ht = __ldg(gp.hop_stats + 1);
             const float cost0 = ((gp.n_chan - 1) * hc + ht) / gp.n_chan;     // mean hop per sample
             const float cost1 = ((gp.tc - 1) * ht + hc) / gp.tc;

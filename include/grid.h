@@ -73,6 +73,25 @@ int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes);
 int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                  const float* conv_kernel, float* grid, grid_stream_t stream);
 
+/* Compression, the step before the path ("merge adjacent visibilities with identical
+ * oversampled position", done as a pre-process and reused for every major cycle; PAPER.md:91 lists what a
+ * compressed sample carries).  Runs a1 and merges every run of consecutive samples with equal
+ * (i0, su, j0, sv, wp) into one pre-weighted sample, in input order; skipped samples (R7) produce none.
+ *   uvw, vis, weights   as for grid_execute (n_vis samples, grid_plan_set_samples)
+ *   out_records  [>= n_vis] 8-byte records (opaque: cell, sub-offsets, plane), DEVICE, 16-byte aligned
+ *   out_vis      [>= n_vis][n_pol] complex64: sum over the run of weights * vis (FP32, input order)
+ *   out_count    DEVICE long long: number of compressed samples written
+ * Needs the plan's workspace.  Power-of-two supports only (GRID_ERR_UNSUPPORTED otherwise). */
+int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                  void* out_records, float* out_vis, long long* out_count, grid_stream_t stream);
+
+/* Grid n compressed samples produced by grid_compress (same plan, n <= the plan's n_vis):
+ *     grid[j0+tj][i0+ti][p] += vis[k][p] * k[wp][sv][tj] * k[wp][su][ti]
+ * i.e. steps a3-a9 of grid_execute on samples that are already quantised and pre-weighted -- the
+ * input the paper's kernel takes.  n is a HOST value (read *out_count back first). */
+int grid_execute_compressed(grid_plan* plan, const void* records, const float* vis, long long n,
+                            const float* conv_kernel, float* grid, grid_stream_t stream);
+
 /* Step a1 alone (the device pass that turns uvw into integer cell, sub-offset and plane index),
  * unpacked for inspection: out is int32 [n][6] = i0, j0, su, sv, wp, valid (invalid: -1 x5, 0).
  * Runs the same device function grid_execute uses.  n need not equal the plan's n_vis. */

@@ -116,3 +116,32 @@ def degrid(grid_size, support, oversample, n_wplanes, n_pol, uvw, weights, kerne
     if rc != 0:
         raise ValueError("oracle_degrid: invalid arguments")
     return out
+
+
+def compress(grid_size, support, oversample, n_wplanes, uvw, vis, weights):
+    """Compression as the paper describes it ("merge adjacent visibilities with identical
+    oversampled position"; a compressed sample carries integer grid coordinates, sub-grid
+    coordinates, w-plane index and pre-weighted values).  Walks the samples in input order; a run is a
+    maximal sequence of CONSECUTIVE valid samples with equal (i0, su, j0, sv, wp); skipped samples (R7)
+    end a run and produce nothing.  Returns (heads int64 [n_c] = index of each run's first sample,
+    merged complex128 [n_c][P] = sum over the run of weight * vis in float64, input order).
+    Test infrastructure only, like everything in oracle/."""
+    q = quantise(grid_size, support, oversample, n_wplanes, uvw)
+    v = np.asarray(vis).reshape(len(q["valid"]), -1)
+    w = np.asarray(weights, dtype=np.float64)
+    heads, merged = [], []
+    prev = None
+    for n in range(len(w)):                           # plain loop: small cases only
+        if not q["valid"][n]:
+            prev = None
+            continue
+        key = (int(q["i0"][n]), int(q["su"][n]), int(q["j0"][n]), int(q["sv"][n]), int(q["wp"][n]))
+        term = w[n] * v[n].astype(np.complex128)
+        if key == prev:
+            merged[-1] = merged[-1] + term
+        else:
+            heads.append(n)
+            merged.append(term)
+            prev = key
+    P = v.shape[1]
+    return np.asarray(heads, dtype=np.int64), np.asarray(merged, dtype=np.complex128).reshape(len(heads), P)

@@ -15,7 +15,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
-    "grid_plan_set_workspace", "grid_execute", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_quantise", "grid_plan_set_tuning",
     "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
@@ -35,6 +35,8 @@ _lib.grid_plan_workspace_bytes.restype = _sz
 _lib.grid_plan_set_workspace.argtypes = [_vp, _vp, _sz]
 _lib.grid_execute.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
+_lib.grid_compress.argtypes = [_vp] * 8
+_lib.grid_execute_compressed.argtypes = [_vp, _vp, _vp, _ll, _vp, _vp, _vp]
 _lib.grid_plan_set_tuning.argtypes = [_vp] + [_int] * 7
 _lib.grid_plan_get_info.argtypes = [_vp, _vp]
 _lib.grid_plan_set_traversal.argtypes = [_vp, _int, _int]
@@ -168,6 +170,31 @@ class GridPlan:
                                _ptr(conv_kernel, torch.complex64, "conv_kernel"),
                                _ptr(grid, torch.complex64, "grid"), _stream(stream))
         _check(rc, "grid_execute")
+
+    def compress(self, uvw, vis, weights, stream=None):
+        """grid_compress: returns (records uint8 [n_c][8], vis complex64 [n_c][P], n_c) -- CUDA tensors trimmed
+        to the compressed count (one host sync to read it)."""
+        import torch
+        n = self.n_vis
+        recs = torch.empty((max(n, 1), 8), dtype=torch.uint8, device=uvw.device)
+        cvis = torch.empty((max(n, 1), self.n_pol), dtype=torch.complex64, device=uvw.device)
+        count = torch.zeros(1, dtype=torch.int64, device=uvw.device)
+        rc = _lib.grid_compress(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
+                                _ptr(weights, torch.float32, "weights"), recs.data_ptr(), cvis.data_ptr(),
+                                count.data_ptr(), _stream(stream))
+        _check(rc, "grid_compress")
+        n_c = int(count.item())
+        return recs[:n_c], cvis[:n_c], n_c
+
+    def execute_compressed(self, records, vis, conv_kernel, grid, stream=None):
+        """grid_execute_compressed on the output of compress()."""
+        import torch
+        n_c = records.shape[0]
+        rc = _lib.grid_execute_compressed(self._h, _ptr(records, torch.uint8, "records") if n_c else None,
+                                          _ptr(vis, torch.complex64, "vis") if n_c else None, n_c,
+                                          _ptr(conv_kernel, torch.complex64, "conv_kernel"),
+                                          _ptr(grid, torch.complex64, "grid"), _stream(stream))
+        _check(rc, "grid_execute_compressed")
 
     def quantise(self, uvw, stream=None):
         """Step a1 alone -> int32 CUDA tensor [n][6] = i0, j0, su, sv, wp, valid."""

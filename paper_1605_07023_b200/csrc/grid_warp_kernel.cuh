@@ -305,7 +305,7 @@ grid_warp_kernel(const GridParams gp) {
             if (k >= count_of(cg, b)) continue;
             const long long g = sample_of(cg, b, k);
             cp_async_8(rrec + kk, recs + g);
-            cp_async_4(rw + kk, gp.weights + g);
+            if (gp.weights) cp_async_4(rw + kk, gp.weights + g);       // null: pre-weighted (compressed) input
             if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
             else {
 #pragma unroll
@@ -344,7 +344,7 @@ grid_warp_kernel(const GridParams gp) {
                 if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
                 else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
                 valid = (rec.pos & 0x8000u) == 0;
-                if (valid) w = rw[kk];
+                if (valid) w = gp.weights ? rw[kk] : 1.f;
             }
             crec[kk] = c;
 #pragma unroll

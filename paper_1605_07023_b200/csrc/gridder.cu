@@ -10,6 +10,7 @@
 #include "grid_kernel.cuh"
 #include "grid_warp_kernel.cuh"
 #include "gridder_common.cuh"
+#include "compress.cuh"
 #include "quantise.cuh"
 
 using namespace gridb200;
@@ -423,38 +424,29 @@ int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid
     return GRID_OK;
 }
 
-int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
-                 const float* conv_kernel, float* grid, grid_stream_t stream_) {
-    cudaStream_t stream = (cudaStream_t)stream_;
-    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute: null plan");
-    plan->last_launches = 0;
-    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute: call grid_plan_set_samples first");
-    if (plan->n_vis == 0) return GRID_OK;                              // R23
-    if (!uvw || !vis || !weights || !conv_kernel || !grid)
-        return fail(GRID_ERR_INVALID_ARG, "grid_execute: null array argument");
-    if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
-        return fail(GRID_ERR_INVALID_ARG, "grid_execute: array arguments must be 16-byte aligned");
-    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
-        return fail(GRID_ERR_STATE, "grid_execute: workspace missing or smaller than grid_plan_workspace_bytes()");
-
+// grid_execute proper.  ext_recs != NULL: the samples are already quantised and pre-weighted (compressed
+// input): no a1 pass, no weights, records read from ext_recs; n_vis samples.
+static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs, long long n_vis, const float* vis,
+                        const float* weights, const float* conv_kernel, float* grid, cudaStream_t stream) {
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
-    SampleRec* recs = reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
+    SampleRec* recs = ext_recs ? reinterpret_cast<SampleRec*>(const_cast<void*>(ext_recs))
+                               : reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
     uint32_t* bins = counters + 64;
-    uint32_t* order = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(recs) + records_bytes(plan));
+    uint32_t* order = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes + records_bytes(plan));
 
     // the layout hint is used only if it is consistent with the sample count
-    const bool have_layout = plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
-                             (long long)plan->n_baselines * plan->n_times * plan->n_channels == plan->n_vis;
+    const bool have_layout = !ext_recs && plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
+                             (long long)plan->n_baselines * plan->n_times * plan->n_channels == n_vis;
     const int n_chan = have_layout ? plan->n_channels : 0, n_times = have_layout ? plan->n_times : 0;
     float* hop_stats = reinterpret_cast<float*>(counters + 2);
 
     // reset the chunk queue and the hop statistics, then a1: quantise pass
     if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
-    {
-        const long long threads = (plan->n_vis + 3) / 4;
+    if (!ext_recs) {
+        const long long threads = (n_vis + 3) / 4;
         const long long blocks = (threads + 255) / 256;
-        quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, plan->n_vis, quant_params(plan), hop_stats,
+        quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, n_vis, quant_params(plan), hop_stats,
                                                              n_chan, n_times, (float)(plan->bin_u + plan->bin_v));
         plan->last_launches++;
     }
@@ -467,7 +459,7 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     gp.kern = reinterpret_cast<const float2*>(conv_kernel);
     gp.grid = grid;
     gp.counters = counters;
-    gp.n_vis = plan->n_vis;
+    gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
     gp.bin_u = plan->bin_u; gp.bin_v = plan->bin_v; gp.row_u = plan->row_u; gp.row_v = plan->row_v;
     gp.nbx = plan->nbx; gp.nby = plan->nby;
@@ -476,7 +468,7 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
 
     if (plan->variant == 0) {
         if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
-        const long long total = plan->n_vis * plan->S;
+        const long long total = n_vis * plan->S;
         const long long blocks = (total + 255) / 256;
         if (blocks > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_execute: too many samples for the scatter variant");
         if (plan->P == 1) grid_scatter_kernel<1><<<(unsigned)blocks, 256, 0, stream>>>(gp);
@@ -492,14 +484,14 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
         const int queues = plan->variant == 3 ? plan->groups_per_cta : 1;               // queue consumers per CTA
         long long want_groups = (long long)plan->n_sm * plan->ctas_per_sm * queues * 4;
         long long per_group = (long long)qt * plan->chunk;
-        if ((plan->n_vis + per_group - 1) / per_group < want_groups) {
-            long long chunk = plan->n_vis / (want_groups * qt);
+        if ((n_vis + per_group - 1) / per_group < want_groups) {
+            long long chunk = n_vis / (want_groups * qt);
             chunk = (chunk + plan->batch - 1) / plan->batch * plan->batch;
             if (chunk < plan->batch) chunk = plan->batch;
             if (chunk < gp.chunk) gp.chunk = (int)chunk;
             per_group = (long long)qt * gp.chunk;
         }
-        gp.n_groups_a = (plan->n_vis + per_group - 1) / per_group;
+        gp.n_groups_a = (n_vis + per_group - 1) / per_group;
         gp.groups_per_cta = plan->groups_per_cta;
         // time-innermost decomposition: chunk = tc time steps x all channels of one baseline
         gp.hop_stats = hop_stats;
@@ -541,7 +533,7 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
         if (plan->variant == 3) {
-            const long long chunks_a = (plan->n_vis + gp.chunk - 1) / gp.chunk;
+            const long long chunks_a = (n_vis + gp.chunk - 1) / gp.chunk;
             const long long max_chunks = chunks_a > gp.n_chunks_b ? chunks_a : gp.n_chunks_b;
             const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
             const bool want = plan->sort_chunks > 0 || (plan->sort_chunks < 0 && grid_bytes > ((size_t)256 << 20));
@@ -571,6 +563,80 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute: launch failed: %s", cudaGetErrorString(e));
     return GRID_OK;
+}
+
+int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                 const float* conv_kernel, float* grid, grid_stream_t stream) {
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute: call grid_plan_set_samples first");
+    if (plan->n_vis == 0) return GRID_OK;                              // R23
+    if (!uvw || !vis || !weights || !conv_kernel || !grid)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute: null array argument");
+    if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute: array arguments must be 16-byte aligned");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_execute: workspace missing or smaller than grid_plan_workspace_bytes()");
+    return execute_impl(plan, uvw, nullptr, plan->n_vis, vis, weights, conv_kernel, grid, (cudaStream_t)stream);
+}
+
+int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const float* weights, void* out_records,
+                  float* out_vis, long long* out_count, grid_stream_t stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_compress: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_compress: call grid_plan_set_samples first");
+    if (plan->variant != 3) return fail(GRID_ERR_UNSUPPORTED, "grid_compress: power-of-two supports (variant 3) only");
+    if (!out_count) return fail(GRID_ERR_INVALID_ARG, "grid_compress: null out_count");
+    if (plan->n_vis == 0) {
+        if (cudaMemsetAsync(out_count, 0, sizeof(long long), stream) != cudaSuccess)
+            return fail(GRID_ERR_CUDA, "grid_compress: %s", cudaGetErrorString(cudaGetLastError()));
+        return GRID_OK;
+    }
+    if (!uvw || !vis || !weights || !out_records || !out_vis)
+        return fail(GRID_ERR_INVALID_ARG, "grid_compress: null array argument");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_compress: workspace missing or smaller than grid_plan_workspace_bytes()");
+    const long long n = plan->n_vis;
+    const long long nb = (n + kCompressBlock - 1) / kCompressBlock;
+    if (nb > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_compress: too many samples");
+    unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
+    unsigned char* rbase = reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes;
+    CycRec* recs = reinterpret_cast<CycRec*>(rbase);                               // 8 B per sample ...
+    uint32_t* block_counts = reinterpret_cast<uint32_t*>(rbase + (size_t)((n + 3) / 4 * 4) * sizeof(CycRec));   // ... the rest of the 16 B
+    if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
+        return fail(GRID_ERR_CUDA, "grid_compress: %s", cudaGetErrorString(cudaGetLastError()));
+    quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
+        uvw, reinterpret_cast<SampleRec*>(recs), n, quant_params(plan), reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
+    compress_count_kernel<<<(unsigned)nb, kCompressBlock, 0, stream>>>(recs, n, block_counts);
+    compress_scan_kernel<<<1, 1024, 0, stream>>>(block_counts, (int)nb, out_count);
+    const float2* v2 = reinterpret_cast<const float2*>(vis);
+    CycRec* orec = reinterpret_cast<CycRec*>(out_records);
+    float2* ovis = reinterpret_cast<float2*>(out_vis);
+    if (plan->P == 1) compress_emit_kernel<1><<<(unsigned)nb, kCompressBlock, 0, stream>>>(recs, v2, weights, n, block_counts, orec, ovis);
+    else if (plan->P == 2) compress_emit_kernel<2><<<(unsigned)nb, kCompressBlock, 0, stream>>>(recs, v2, weights, n, block_counts, orec, ovis);
+    else compress_emit_kernel<4><<<(unsigned)nb, kCompressBlock, 0, stream>>>(recs, v2, weights, n, block_counts, orec, ovis);
+    plan->last_launches = 4;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_compress: launch failed: %s", cudaGetErrorString(e));
+    return GRID_OK;
+}
+
+int grid_execute_compressed(grid_plan* plan, const void* records, const float* vis, long long n,
+                            const float* conv_kernel, float* grid, grid_stream_t stream) {
+    if (!plan || n < 0) return fail(GRID_ERR_INVALID_ARG, "grid_execute_compressed: invalid argument");
+    plan->last_launches = 0;
+    if (plan->variant != 3) return fail(GRID_ERR_UNSUPPORTED, "grid_execute_compressed: power-of-two supports (variant 3) only");
+    if (plan->n_vis < 0 || n > plan->n_vis)
+        return fail(GRID_ERR_STATE, "grid_execute_compressed: set_samples must cover the uncompressed count (workspace size)");
+    if (n == 0) return GRID_OK;
+    if (!records || !vis || !conv_kernel || !grid)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_compressed: null array argument");
+    if ((((uintptr_t)records | (uintptr_t)vis | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_compressed: array arguments must be 16-byte aligned");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_execute_compressed: workspace missing or too small");
+    return execute_impl(plan, nullptr, records, n, vis, nullptr, conv_kernel, grid, (cudaStream_t)stream);
 }
 
 }  // extern "C"

@@ -338,3 +338,43 @@ def test_quantise_matches_independent_python(oracle_mod):
             else:
                 assert q["valid"][k] == 0
             assert j_ok or q["valid"][k] == 0
+
+
+def test_compress_oracle_runs_and_invariance(oracle_mod):
+    # oracle.compress against what its definition fixes: hand-built runs, and the grid of the
+    # compressed samples equals the grid of the originals (values chosen exactly representable in float32)
+    rng = np.random.default_rng(21)
+    base = rng.uniform(-10, 10, (40, 3)).astype(np.float32)
+    base[:, 2] = rng.uniform(0, W, 40)
+    reps = rng.integers(1, 5, 40)
+    uvw = np.repeat(base, reps, axis=0)
+    uvw[7] = np.nan                                           # a skipped sample splits / removes a run
+    n = len(uvw)
+    vis = (rng.integers(-8, 9, (n, 2)) + 1j * rng.integers(-8, 9, (n, 2))).astype(np.complex64)
+    wts = rng.integers(1, 4, n).astype(np.float32)
+    heads, merged = oracle_mod.compress(N, S, O, W, uvw, vis, wts)
+    # expected run heads straight from the construction: one per repeated position, except around the NaN
+    starts = np.concatenate([[0], np.cumsum(reps)[:-1]])
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    expect = []
+    for s0, r in zip(starts, reps):
+        idx = [m for m in range(s0, s0 + r) if q["valid"][m]]
+        # consecutive valid members form runs; the NaN at 7 may split one
+        run = []
+        for m in idx:
+            if run and m != run[-1] + 1:
+                expect.append(run); run = []
+            run.append(m)
+        if run:
+            expect.append(run)
+    # neighbouring base positions may coincide after quantisation only by accident; rule that out
+    keys = [(q["i0"][r[0]], q["su"][r[0]], q["j0"][r[0]], q["sv"][r[0]], q["wp"][r[0]]) for r in expect]
+    assert all(keys[k] != keys[k + 1] or expect[k][-1] + 1 != expect[k + 1][0] for k in range(len(keys) - 1))
+    assert list(heads) == [r[0] for r in expect]
+    for k, r in enumerate(expect):
+        np.testing.assert_array_equal(merged[k], sum(float(wts[m]) * vis[m].astype(np.complex128) for m in r))
+    # invariance ("identical results"): merged values are small integers, exact in complex64
+    g = oracle_mod.grid(N, S, O, W, 2, uvw, vis, wts, np.ones((W, O, S), np.complex64) * (1 + 0.5j))
+    g_c = oracle_mod.grid(N, S, O, W, 2, uvw[heads], merged.astype(np.complex64), np.ones(len(heads), np.float32),
+                          np.ones((W, O, S), np.complex64) * (1 + 0.5j))
+    np.testing.assert_allclose(g_c, g, rtol=1e-12, atol=1e-12)

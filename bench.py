@@ -38,6 +38,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--compressed", action="store_true",
+                    help="compress once outside the timed region (PAPER.md:69, 113) and time grid_execute_compressed; "
+                         "the rate then counts compressed samples, as the paper's does")
     ap.add_argument("--tuning", default="", help="e.g. cu=2,cv=2,threads_per_cta=256")
     return ap.parse_args()
 
@@ -235,6 +238,22 @@ def run_ours(args):
     n_valid = int(q[:, 5].sum().item())
     del q
     updates_per_step = n_valid * S * S * P
+    compressed = None
+    if args.compressed:
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        plan.compress(d_uvw, d_vis, d_wts)                      # warm-up
+        c0.record()
+        c_recs, c_vis, n_c = plan.compress(d_uvw, d_vis, d_wts)
+        c1.record()
+        torch.cuda.synchronize()
+        compressed = {"n_compressed": n_c, "ratio": cfg.n_vis / max(n_c, 1), "compress_ms": c0.elapsed_time(c1)}
+        updates_per_step = n_c * S * S * P
+
+    def step():
+        if compressed:
+            plan.execute_compressed(c_recs, c_vis, d_kern, grid)
+        else:
+            plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
 
     def barrier():
         if world > 1:
@@ -243,7 +262,7 @@ def run_ours(args):
 
     stream = torch.cuda.current_stream()
     for _ in range(max(args.warmup, 3)):
-        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        step()
     barrier()
 
     # ---- device-resident timing: exactly K steps, CUDA events on the launching stream
@@ -260,7 +279,7 @@ def run_ours(args):
     ev0.record(stream)
     for k in range(args.steps):
         plan.set_kernel_events(*k_events[k])
-        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        step()
         launches += plan.last_launches()
     ev1.record(stream)
     barrier()
@@ -271,7 +290,7 @@ def run_ours(args):
 
     # ---- end to end: pinned host inputs -> device, execute, grid -> pinned host, every step
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not compressed:
         h_grid = torch.empty((N, N, P), dtype=torch.complex64).pin_memory()
         e_steps = max(3, min(args.steps, 10))
         h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4
@@ -307,7 +326,7 @@ def run_ours(args):
                        "oversample": O, "n_wplanes": W, "n_pol": P, "updates_per_step": updates_per_step,
                        "l2": "inputs (%.2f GB per step) exceed the 126 MB L2; no explicit flush" %
                              ((h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4) / 1e9),
-                       "tuning": info},
+                       "tuning": info, "compressed": compressed},
             "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_FP32_TFLOPS, "traffic": ncu_traffic(cfg.name),

@@ -92,6 +92,15 @@ int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const flo
 int grid_execute_compressed(grid_plan* plan, const void* records, const float* vis, long long n,
                             const float* conv_kernel, float* grid, grid_stream_t stream);
 
+/* Degridding, the adjoint of grid_execute (the paper calls its own degridder preliminary
+ * and does not measure it).  For every sample whose footprint lies inside the grid
+ *     vis_out[n][p] = weights[n] * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * grid[j0+tj][i0+ti][p]
+ * with the same Q, W as grid_execute; skipped samples (R7) get zeros.  <grid_execute(V), G> equals
+ * <V, grid_degrid(G)> (pin P7).  grid is read-only; vis_out [n_vis][n_pol] complex64 is overwritten.
+ * First version: a gather kernel bound by L2 bandwidth; any support. */
+int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const float* conv_kernel,
+                const float* grid, float* vis_out, grid_stream_t stream);
+
 /* Step a1 alone (the device pass that turns uvw into integer cell, sub-offset and plane index),
  * unpacked for inspection: out is int32 [n][6] = i0, j0, su, sv, wp, valid (invalid: -1 x5, 0).
  * Runs the same device function grid_execute uses.  n need not equal the plan's n_vis. */

@@ -11,6 +11,7 @@
 #include "grid_warp_kernel.cuh"
 #include "gridder_common.cuh"
 #include "compress.cuh"
+#include "degrid_kernel.cuh"
 #include "quantise.cuh"
 
 using namespace gridb200;
@@ -279,6 +280,15 @@ QuantParams quant_params(const grid_plan* p) {
 }
 
 }  // namespace
+
+template <int P>
+static void launch_degrid(int L, long long n, const CycRec* recs, const float* weights, const float2* kern,
+                          const float2* grid, float2* out, int N, int S, cudaStream_t stream) {
+    const unsigned blocks = (unsigned)((n * L + 255) / 256);
+    if (L == 8) degrid_gather_kernel<P, 8><<<blocks, 256, 0, stream>>>(recs, weights, kern, grid, out, n, N, S);
+    else if (L == 16) degrid_gather_kernel<P, 16><<<blocks, 256, 0, stream>>>(recs, weights, kern, grid, out, n, N, S);
+    else degrid_gather_kernel<P, 32><<<blocks, 256, 0, stream>>>(recs, weights, kern, grid, out, n, N, S);
+}
 
 extern "C" {
 
@@ -619,6 +629,44 @@ int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const flo
     plan->last_launches = 4;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_compress: launch failed: %s", cudaGetErrorString(e));
+    return GRID_OK;
+}
+
+int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const float* conv_kernel,
+                const float* grid, float* vis_out, grid_stream_t stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_degrid: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_degrid: call grid_plan_set_samples first");
+    if (plan->n_vis == 0) return GRID_OK;
+    if (!uvw || !weights || !conv_kernel || !grid || !vis_out)
+        return fail(GRID_ERR_INVALID_ARG, "grid_degrid: null array argument");
+    if ((((uintptr_t)uvw | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid | (uintptr_t)vis_out) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_degrid: array arguments must be 16-byte aligned");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_degrid: workspace missing or smaller than grid_plan_workspace_bytes()");
+    const long long n = plan->n_vis;
+    if (n * 32 / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_degrid: too many samples");
+    unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
+    CycRec* recs = reinterpret_cast<CycRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
+    if (cudaMemsetAsync(counters, 0, 256, stream) != cudaSuccess)
+        return fail(GRID_ERR_CUDA, "grid_degrid: %s", cudaGetErrorString(cudaGetLastError()));
+    QuantParams qp = quant_params(plan);
+    qp.format = 1;                                   // compact records (cell, tap rows) for every support
+    quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
+        uvw, reinterpret_cast<SampleRec*>(recs), n, qp, reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
+    const int L = plan->S <= 8 ? 8 : (plan->S <= 16 ? 16 : 32);
+    const float2* k2 = reinterpret_cast<const float2*>(conv_kernel);
+    const float2* g2 = reinterpret_cast<const float2*>(grid);
+    float2* o2 = reinterpret_cast<float2*>(vis_out);
+    if (plan->ev_start) cudaEventRecord(plan->ev_start, stream);
+    if (plan->P == 1) launch_degrid<1>(L, n, recs, weights, k2, g2, o2, plan->N, plan->S, stream);
+    else if (plan->P == 2) launch_degrid<2>(L, n, recs, weights, k2, g2, o2, plan->N, plan->S, stream);
+    else launch_degrid<4>(L, n, recs, weights, k2, g2, o2, plan->N, plan->S, stream);
+    if (plan->ev_stop) cudaEventRecord(plan->ev_stop, stream);
+    plan->last_launches = 2;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_degrid: launch failed: %s", cudaGetErrorString(e));
     return GRID_OK;
 }
 

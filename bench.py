@@ -38,6 +38,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--op", default="grid", choices=["grid", "degrid"],
+                    help="degrid: time grid_degrid (the adjoint, SURVEY NEXT-2) instead of grid_execute")
     ap.add_argument("--compressed", action="store_true",
                     help="compress once outside the timed region (PAPER.md:69, 113) and time grid_execute_compressed; "
                          "the rate then counts compressed samples, as the paper's does")
@@ -249,8 +251,15 @@ def run_ours(args):
         compressed = {"n_compressed": n_c, "ratio": cfg.n_vis / max(n_c, 1), "compress_ms": c0.elapsed_time(c1)}
         updates_per_step = n_c * S * S * P
 
+    d_out = torch.empty((cfg.n_vis, P), dtype=torch.complex64, device=dev) if args.op == "degrid" else None
+    if d_out is not None:                                      # a non-trivial grid to read from
+        grid.copy_(torch.randn((N, N, P), dtype=torch.complex64, device=dev))
+        kernel_name = "degrid_gather_kernel<%d>" % P
+
     def step():
-        if compressed:
+        if d_out is not None:
+            plan.degrid(d_uvw, d_wts, d_kern, grid, d_out)
+        elif compressed:
             plan.execute_compressed(c_recs, c_vis, d_kern, grid)
         else:
             plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
@@ -290,7 +299,7 @@ def run_ours(args):
 
     # ---- end to end: pinned host inputs -> device, execute, grid -> pinned host, every step
     e2e = None
-    if not args.no_e2e and not compressed:
+    if not args.no_e2e and not compressed and d_out is None:
         h_grid = torch.empty((N, N, P), dtype=torch.complex64).pin_memory()
         e_steps = max(3, min(args.steps, 10))
         h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4
@@ -326,7 +335,7 @@ def run_ours(args):
                        "oversample": O, "n_wplanes": W, "n_pol": P, "updates_per_step": updates_per_step,
                        "l2": "inputs (%.2f GB per step) exceed the 126 MB L2; no explicit flush" %
                              ((h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4) / 1e9),
-                       "tuning": info, "compressed": compressed},
+                       "tuning": info, "compressed": compressed, "op": args.op},
             "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_FP32_TFLOPS, "traffic": ncu_traffic(cfg.name),

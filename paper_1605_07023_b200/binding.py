@@ -15,7 +15,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
-    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_degrid", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
     "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
@@ -37,6 +37,7 @@ _lib.grid_execute.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
 _lib.grid_compress.argtypes = [_vp] * 8
 _lib.grid_degrid.argtypes = [_vp] * 7
+_lib.grid_plan_set_degrid_gather.argtypes = [_vp, _int]
 _lib.grid_execute_compressed.argtypes = [_vp, _vp, _vp, _ll, _vp, _vp, _vp]
 _lib.grid_plan_set_tuning.argtypes = [_vp] + [_int] * 7
 _lib.grid_plan_get_info.argtypes = [_vp, _vp]
@@ -196,6 +197,9 @@ class GridPlan:
                                           _ptr(conv_kernel, torch.complex64, "conv_kernel"),
                                           _ptr(grid, torch.complex64, "grid"), _stream(stream))
         _check(rc, "grid_execute_compressed")
+
+    def set_degrid_gather(self, on=1):
+        _check(_lib.grid_plan_set_degrid_gather(self._h, on), "grid_plan_set_degrid_gather")
 
     def degrid(self, uvw, weights, conv_kernel, grid, vis_out=None, stream=None):
         """grid_degrid: vis_out complex64 [n][P] (allocated if None) = adjoint of execute() applied to grid."""

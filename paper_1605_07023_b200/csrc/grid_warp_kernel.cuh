@@ -93,7 +93,11 @@ struct WarpKernelTraits {
     }
 };
 
-template <int CU, int CV, int P, int LOGS, int PS = 1>
+// DEGRID: the same ownership, staging and traversal run backwards: the
+// registers hold the VALUES of the owned grid points (loaded when the footprint moves onto a new point,
+// where gridding flushes), every sample takes sum conj(G_ij) * value over the owned points, a shuffle
+// tree adds the team's partial sums and one lane stores weight * sum to vis_out.  No atomics.
+template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false>
 __global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS, PS>::MAX_THREADS), 1)
 grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
@@ -102,6 +106,7 @@ grid_warp_kernel(const GridParams gp) {
     constexpr int ROW = 2 * S;                         // doubled tap row k[t mod S], t < 2S: offsets reach 2S-1
     constexpr bool WIDE = S > 16;                      // record format: 32-bit masks need two words
     static_assert(CU <= S && CV <= S, "block larger than the support");
+    static_assert(!DEGRID || T::TEAM <= 32, "degridding: a team must fit one warp (shuffle reduction)");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* taps = reinterpret_cast<float2*>(smem_raw);
@@ -145,7 +150,7 @@ grid_warp_kernel(const GridParams gp) {
     for (int b = 0; b < CV; ++b) MY |= 1u << (s0 + b * DV);
     const uint32_t MXY = MX | (MY << 16);              // !WIDE: both masks in one word
     const uint4* my_rec = crec + (size_t)tg * B;
-    const float2* my_vis = cvis + (size_t)tg * B * P + half * PT;
+    const float2* my_vis = cvis + (size_t)tg * B * P + (DEGRID ? 0 : half * PT);   // DEGRID: {weight, sample code}
     const unsigned char* my_tu = reinterpret_cast<const unsigned char*>(taps + r0);
     const unsigned char* my_tv = reinterpret_cast<const unsigned char*>(taps + s0);
     const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
@@ -174,6 +179,21 @@ grid_warp_kernel(const GridParams gp) {
     auto clear_point = [&](float2 (&v)[PT]) {
 #pragma unroll
         for (int q = 0; q < PT; ++q) v[q] = make_float2(0.f, 0.f);
+    };
+
+    // DEGRID: fetch the value of a grid point my team now covers
+    auto load_point = [&](float2 (&v)[PT], uint32_t cell) {
+        const float* p = gridp + (size_t)cell * (2 * P) + half * (2 * PT);
+        if constexpr (PT == 4) {
+            const float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
+            v[0] = make_float2(a.x, a.y); v[1] = make_float2(a.z, a.w);
+            v[2] = make_float2(b.x, b.y); v[3] = make_float2(b.z, b.w);
+        } else if constexpr (PT == 2) {
+            const float4 a = *reinterpret_cast<const float4*>(p);
+            v[0] = make_float2(a.x, a.y); v[1] = make_float2(a.z, a.w);
+        } else {
+            v[0] = *reinterpret_cast<const float2*>(p);
+        }
     };
 
     // a8: one grid point, all polarisations: atomic add, then clear
@@ -293,6 +313,10 @@ grid_warp_kernel(const GridParams gp) {
         return cg.base + (long long)ti * gp.n_chan + col;
     };
 
+    // DEGRID: sample indices are kept as 31-bit offsets from here (a mirrored time row of the
+    // channel-innermost walk reaches back to the start of its row, before the chunk's first position)
+    auto out_base = [&](const WarpChunk& cg) -> long long { return mode == 0 ? cg.base - cg.col0 : cg.base; };
+
     // a3: start the copies of batch b of the chunk group `par` into raw stage `st`
     auto issue = [&](int par, int b, int st) {
         unsigned char* rs = rbase + (size_t)st * rstage;
@@ -306,7 +330,8 @@ grid_warp_kernel(const GridParams gp) {
             const long long g = sample_of(cg, b, k);
             cp_async_8(rrec + kk, recs + g);
             if (gp.weights) cp_async_4(rw + kk, gp.weights + g);       // null: pre-weighted (compressed) input
-            if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
+            if constexpr (DEGRID) {
+            } else if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
             else {
 #pragma unroll
                 for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + g * P + q);
@@ -347,11 +372,18 @@ grid_warp_kernel(const GridParams gp) {
                 if (valid) w = gp.weights ? rw[kk] : 1.f;
             }
             crec[kk] = c;
+            if constexpr (DEGRID) {
+                // where the result goes: offset from the chunk base, bit 31 = skipped sample, all ones = no sample
+                uint32_t code = 0xffffffffu;
+                if (k < cnt) code = (uint32_t)(sample_of(cg, b, k) - out_base(cg)) | (valid ? 0u : 0x80000000u);
+                cvis[(size_t)kk * P] = make_float2(w, __uint_as_float(code));
+            } else {
 #pragma unroll
-            for (int q = 0; q < P; ++q) {
-                float2 v = make_float2(0.f, 0.f);
-                if (valid) { v = rvis[(size_t)kk * P + q]; v.x *= w; v.y *= w; }
-                cvis[(size_t)kk * P + q] = v;
+                for (int q = 0; q < P; ++q) {
+                    float2 v = make_float2(0.f, 0.f);
+                    if (valid) { v = rvis[(size_t)kk * P + q]; v.x *= w; v.y *= w; }
+                    cvis[(size_t)kk * P + q] = v;
+                }
             }
         }
     };
@@ -388,6 +420,12 @@ grid_warp_kernel(const GridParams gp) {
                 for (int a = 0; a < CU; ++a) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
 #pragma unroll
                 for (int bb = 0; bb < CV; ++bb) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                if constexpr (DEGRID) {
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                        for (int a = 0; a < CU; ++a) load_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                }
             }
             if constexpr (TPG > 1) cnt = __reduce_max_sync(0xffffffffu, cnt);
 
@@ -404,6 +442,30 @@ grid_warp_kernel(const GridParams gp) {
                     const int i0 = (int)(c.x & 0x7fffu), j0 = (int)(c.x >> 16);
                     const uint32_t mxs = (WIDE ? c.z : c.w) >> r0;
                     const uint32_t mys = (WIDE ? c.w : (c.w >> 16)) >> s0;
+                    if constexpr (DEGRID) {
+                        // positions first, then the values of every point that changed (a point whose
+                        // column AND row moved is fetched twice; harmless)
+#pragma unroll
+                        for (int a = 0; a < CU; ++a)
+                            if (mxs & (1u << (a * DU))) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+#pragma unroll
+                        for (int bb = 0; bb < CV; ++bb)
+                            if (mys & (1u << (bb * DV))) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+#pragma unroll
+                        for (int a = 0; a < CU; ++a) {
+                            if (mxs & (1u << (a * DU))) {
+#pragma unroll
+                                for (int bb = 0; bb < CV; ++bb) load_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                            }
+                        }
+#pragma unroll
+                        for (int bb = 0; bb < CV; ++bb) {
+                            if (mys & (1u << (bb * DV))) {
+#pragma unroll
+                                for (int a = 0; a < CU; ++a) load_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
+                            }
+                        }
+                    } else {
 #pragma unroll
                     for (int a = 0; a < CU; ++a) {
                         if (mxs & (1u << (a * DU))) {  // owned column a left the footprint
@@ -421,6 +483,7 @@ grid_warp_kernel(const GridParams gp) {
                             ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
                         }
                     }
+                    }
                 }
                 const float2* tu;
                 const float2* tv;
@@ -436,6 +499,49 @@ grid_warp_kernel(const GridParams gp) {
                 for (int a = 0; a < CU; ++a) gu[a] = tu[a * DU];
 #pragma unroll
                 for (int bb = 0; bb < CV; ++bb) gv[bb] = tv[bb * DV];
+                if constexpr (DEGRID) {
+                    // sum over my points of conj(Gv_j * Gu_i) * value: rows first (conj(Gu_i) * value), then conj(Gv_j)
+                    const float2 meta = *vp;                   // {weight, where the result goes}
+                    vp += P;
+                    float2 part[PT];
+#pragma unroll
+                    for (int q = 0; q < PT; ++q) part[q] = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb) {
+#pragma unroll
+                        for (int q = 0; q < PT; ++q) {
+                            float rx = 0.f, ry_ = 0.f;
+#pragma unroll
+                            for (int a = 0; a < CU; ++a) {
+                                rx = fmaf(gu[a].x, acc[bb][a][q].x, rx);
+                                rx = fmaf(gu[a].y, acc[bb][a][q].y, rx);
+                                ry_ = fmaf(gu[a].x, acc[bb][a][q].y, ry_);
+                                ry_ = fmaf(-gu[a].y, acc[bb][a][q].x, ry_);
+                            }
+                            part[q].x = fmaf(gv[bb].x, rx, part[q].x);
+                            part[q].x = fmaf(gv[bb].y, ry_, part[q].x);
+                            part[q].y = fmaf(gv[bb].x, ry_, part[q].y);
+                            part[q].y = fmaf(-gv[bb].y, rx, part[q].y);
+                        }
+                    }
+#pragma unroll
+                    for (int o = PS; o < TEAM; o <<= 1) {      // the team's lanes are adjacent and aligned
+#pragma unroll
+                        for (int q = 0; q < PT; ++q) {
+                            part[q].x += __shfl_xor_sync(0xffffffffu, part[q].x, o);
+                            part[q].y += __shfl_xor_sync(0xffffffffu, part[q].y, o);
+                        }
+                    }
+                    const uint32_t code = __float_as_uint(meta.y);
+                    if (ct == 0 && code != 0xffffffffu) {
+                        float2* o = gp.vis_out + (out_base(my_cg) + (long long)(code & 0x7fffffffu)) * P + half * PT;
+                        const float w = (code >> 31) ? 0.f : meta.x;
+#pragma unroll
+                        for (int q = 0; q < PT; ++q)
+                            o[q] = (code >> 31) ? make_float2(0.f, 0.f) : make_float2(w * part[q].x, w * part[q].y);
+                    }
+                    continue;
+                }
                 if constexpr (PT == 4) {
                     const float4 v01 = *reinterpret_cast<const float4*>(vp);
                     const float4 v23 = *reinterpret_cast<const float4*>(vp + 2);
@@ -484,7 +590,7 @@ grid_warp_kernel(const GridParams gp) {
                 }
             }
         }
-        if (live) {                                    // end of chunk: everything goes to the grid
+        if (live && !DEGRID) {                         // end of chunk: everything goes to the grid
 #pragma unroll
             for (int bb = 0; bb < CV; ++bb)
 #pragma unroll

@@ -44,6 +44,7 @@ struct grid_plan {
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
     int groups_per_cta, queue_teams;
+    int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
     int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on      // variant 3: warp groups per CTA; teams per queue entry (all variants)
     int n_sm, max_smem;
@@ -104,6 +105,27 @@ WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps) {
     CASE(2, 2, 4, 2) CASE(4, 2, 4, 2) CASE(4, 4, 4, 2) CASE(2, 1, 4, 2)
 #undef CASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+// Coarsened degridding kernels (grid_warp_kernel<..., DEGRID = true>): teams of at most one warp.
+template <int CU, int CV, int P>
+kernel_fn pick_degrid(int logs) {
+    switch (logs) {
+        case 2: if constexpr (WarpKernelTraits<CU, CV, P, 2>::TEAM <= 32 && CU <= 4 && CV <= 4) return grid_warp_kernel<CU, CV, P, 2, 1, true>; break;
+        case 3: if constexpr (WarpKernelTraits<CU, CV, P, 3>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 3, 1, true>; break;
+        case 4: if constexpr (WarpKernelTraits<CU, CV, P, 4>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 4, 1, true>; break;
+        case 5: if constexpr (WarpKernelTraits<CU, CV, P, 5>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 5, 1, true>; break;
+    }
+    return nullptr;
+}
+
+kernel_fn lookup_degrid(int cu, int cv, int P, int logs) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_degrid<a, b, p>(logs);
+    CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
+    CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
+    CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+    return nullptr;
 }
 
 int log2_exact(int v) {
@@ -406,6 +428,12 @@ int grid_plan_set_pol_split(grid_plan* plan, int lanes) {
     return GRID_OK;
 }
 
+int grid_plan_set_degrid_gather(grid_plan* plan, int on) {
+    if (!plan || (on != 0 && on != 1)) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_degrid_gather: on in {0,1}");
+    plan->degrid_gather = on;
+    return GRID_OK;
+}
+
 int grid_plan_set_chunk_order(grid_plan* plan, int mode) {
     if (!plan || mode < -1 || mode > 1)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_chunk_order: mode in {-1,0,1}");
@@ -436,8 +464,11 @@ int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid
 
 // grid_execute proper.  ext_recs != NULL: the samples are already quantised and pre-weighted (compressed
 // input): no a1 pass, no weights, records read from ext_recs; n_vis samples.
+// degrid_out != NULL: run the DEGRID kernel (grid is read, degrid_out written; plan must be variant 3,
+// pol split 1, team <= 32 -- the caller checks with lookup_degrid).
 static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs, long long n_vis, const float* vis,
-                        const float* weights, const float* conv_kernel, float* grid, cudaStream_t stream) {
+                        const float* weights, const float* conv_kernel, float* grid, cudaStream_t stream,
+                        float* degrid_out = nullptr) {
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
     SampleRec* recs = ext_recs ? reinterpret_cast<SampleRec*>(const_cast<void*>(ext_recs))
                                : reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
@@ -468,6 +499,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.weights = weights;
     gp.kern = reinterpret_cast<const float2*>(conv_kernel);
     gp.grid = grid;
+    gp.vis_out = reinterpret_cast<float2*>(degrid_out);
     gp.counters = counters;
     gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
@@ -539,7 +571,8 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);
-        kernel_fn fn = plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
+        kernel_fn fn = degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs)
+                     : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
         if (plan->variant == 3) {
@@ -645,6 +678,11 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
         return fail(GRID_ERR_INVALID_ARG, "grid_degrid: array arguments must be 16-byte aligned");
     if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
         return fail(GRID_ERR_STATE, "grid_degrid: workspace missing or smaller than grid_plan_workspace_bytes()");
+    // the coarsened, register-resident kernel where the plan offers one; the gather kernel otherwise
+    if (plan->variant == 3 && plan->pol_split == 1 && plan->degrid_gather == 0 &&
+        lookup_degrid(plan->cu, plan->cv, plan->P, log2_exact(plan->S)))
+        return execute_impl(plan, uvw, nullptr, plan->n_vis, nullptr, weights, conv_kernel, const_cast<float*>(grid),
+                            stream, vis_out);
     const long long n = plan->n_vis;
     if (n * 32 / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_degrid: too many samples");
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);

@@ -37,6 +37,7 @@ struct GridParams {
     const float* weights;     // [n_vis]
     const float2* kern;       // [W][O][S]
     float* grid;              // [N][N][P] complex64
+    float2* vis_out;          // degridding only: [n_vis][P] complex64 result
     unsigned int* counters;   // [0]: next chunk group
     const float* hop_stats;   // [0] mean-hop sum along channels, [1] along time (quantise pass)
     long long n_vis;

@@ -9,7 +9,7 @@ from gpu_util import run_gpu
 pytestmark = pytest.mark.gpu
 
 
-def gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid):
+def gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid, layout=None, tuning=None, gather=False):
     import torch
     from paper_1605_07023_b200 import binding
     dev = torch.device("cuda:0")
@@ -17,6 +17,15 @@ def gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid):
     try:
         n = uvw.shape[0]
         plan.set_samples(n)
+        if layout:
+            plan.set_layout(*layout)
+        if tuning:
+            tuning = dict(tuning)
+            if "traversal" in tuning:
+                plan.set_traversal(tuning.pop("traversal"), tuning.pop("time_block", 0))
+            plan.set_tuning(**tuning)
+        if gather:
+            plan.set_degrid_gather(1)
         plan.allocate_workspace(dev)
         out = plan.degrid(torch.from_numpy(uvw).to(dev), torch.from_numpy(wts).to(dev),
                           torch.from_numpy(kernel).to(dev), torch.from_numpy(grid.astype(np.complex64)).to(dev))
@@ -57,3 +66,30 @@ def test_adjoint_identity_on_gpu(oracle_mod):
     lhs = np.vdot(gv.astype(np.complex128), G.astype(np.complex128))
     rhs = np.vdot(vis.astype(np.complex128), dg.astype(np.complex128))
     assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
+
+
+@pytest.mark.parametrize("cu,cv,P,S", [(2, 2, 4, 8), (4, 2, 4, 8), (2, 1, 4, 8), (4, 4, 1, 16), (4, 2, 1, 8), (2, 2, 1, 4),
+                                       (8, 4, 1, 32), (4, 4, 2, 16), (2, 2, 2, 8), (8, 4, 1, 16)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_degrid_coarsened_blocks(oracle_mod, cu, cv, P, S, mode):
+    # the register-resident kernel (ownership of PAPER.md:63, 77-87 run backwards) for every instantiated
+    # block, both traversal orders, small chunks and batches, against the oracle AND the gather kernel
+    cfg = synth.shrink(synth.get_config("cfg1"), n_ant=9, n_times=37, n_chan=13, grid_size=384)
+    rng = np.random.default_rng(cu * 10 + cv)
+    uvw = synth.make_uvw(cfg, rng)
+    uvw[50:60, 1] = np.nan
+    n = uvw.shape[0]
+    N, O, W = cfg.grid_size, 4, 3
+    uvw[:, 2] = rng.uniform(0, W, n)
+    wts = rng.uniform(0.5, 1.0, n).astype(np.float32)
+    kernel = (rng.standard_normal((W, O, S)) + 1j * rng.standard_normal((W, O, S))).astype(np.complex64)
+    grid = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+    ref = oracle_mod.degrid(N, S, O, W, P, uvw, wts, kernel, grid)
+    layout = (cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    tuning = dict(variant=3, cu=cu, cv=cv, threads_per_cta=1024, batch=16, chunk=64, traversal=mode, time_block=8)
+    got = gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid, layout=layout, tuning=tuning).astype(np.complex128)
+    via_gather = gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid, gather=True).astype(np.complex128)
+    assert np.linalg.norm(got - ref) <= 1e-5 * np.linalg.norm(ref)
+    assert np.abs(got - ref).max() <= 2e-5 * np.sqrt(np.mean(np.abs(ref) ** 2)) * max(1.0, S / 8)
+    assert np.linalg.norm(got - via_gather) <= 2e-5 * np.linalg.norm(ref)
+    assert not got[50:60].any()

@@ -254,7 +254,7 @@ def run_ours(args):
     d_out = torch.empty((cfg.n_vis, P), dtype=torch.complex64, device=dev) if args.op == "degrid" else None
     if d_out is not None:                                      # a non-trivial grid to read from
         grid.copy_(torch.randn((N, N, P), dtype=torch.complex64, device=dev))
-        kernel_name = "degrid_gather_kernel<%d>" % P
+        kernel_name = "grid_degrid: grid_warp_kernel<..,DEGRID> where a team fits a warp, else degrid_gather_kernel"
 
     def step():
         if d_out is not None:

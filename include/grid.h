@@ -103,6 +103,7 @@ int grid_execute_compressed(grid_plan* plan, const void* records, const float* v
 int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const float* conv_kernel,
                 const float* grid, float* vis_out, grid_stream_t stream);
 
+/* on = 1: grid_degrid always uses the gather kernel (diagnostic / comparison); 0 = automatic (default). */
 int grid_plan_set_degrid_gather(grid_plan* plan, int on);
 
 /* Step a1 alone (the device pass that turns uvw into integer cell, sub-offset and plane index),

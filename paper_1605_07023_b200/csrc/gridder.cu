@@ -679,10 +679,23 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
     if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
         return fail(GRID_ERR_STATE, "grid_degrid: workspace missing or smaller than grid_plan_workspace_bytes()");
     // the coarsened, register-resident kernel where the plan offers one; the gather kernel otherwise
-    if (plan->variant == 3 && plan->pol_split == 1 && plan->degrid_gather == 0 &&
-        lookup_degrid(plan->cu, plan->cv, plan->P, log2_exact(plan->S)))
-        return execute_impl(plan, uvw, nullptr, plan->n_vis, nullptr, weights, conv_kernel, const_cast<float*>(grid),
-                            stream, vis_out);
+    if (plan->variant == 3 && plan->degrid_gather == 0) {
+        grid_plan tmp = *plan;                       // same plan with polarisation split 1 (shuffle reduction per team)
+        tmp.pol_split = 1;
+        tmp.threads = 1024;
+        const int logs = log2_exact(plan->S);
+        const int tries[3][2] = {{plan->cu, plan->cv}, {4, 2}, {2, 2}};
+        for (int t = 0; t < 3; ++t) {
+            tmp.cu = tries[t][0]; tmp.cv = tries[t][1];
+            if (lookup_degrid(tmp.cu, tmp.cv, tmp.P, logs) && derive(&tmp) == GRID_OK) {
+                const int rc = execute_impl(&tmp, uvw, nullptr, plan->n_vis, nullptr, weights, conv_kernel,
+                                            const_cast<float*>(grid), stream, vis_out);
+                plan->last_launches = tmp.last_launches;
+                return rc;
+            }
+        }
+        g_err[0] = 0;                                // no coarsened kernel for this shape: gather below
+    }
     const long long n = plan->n_vis;
     if (n * 32 / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_degrid: too many samples");
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);

@@ -524,21 +524,43 @@ grid_warp_kernel(const GridParams gp) {
                             part[q].y = fmaf(-gv[bb].y, rx, part[q].y);
                         }
                     }
+                    // Team sum by recursive halving (the team's lanes are adjacent and aligned): at each step a
+                    // lane keeps one half of its values and hands the other half to its partner, so the 2*PT
+                    // floats end up spread over the lanes -- 2*PT-1 shuffles and adds instead of 2*PT*log2(TEAM).
+                    float val[2 * PT];
 #pragma unroll
-                    for (int o = PS; o < TEAM; o <<= 1) {      // the team's lanes are adjacent and aligned
+                    for (int q = 0; q < PT; ++q) { val[2 * q] = part[q].x; val[2 * q + 1] = part[q].y; }
+                    int first = 0;                             // my values are floats [first, first + width) of the result
+                    constexpr int W0 = 2 * PT;
+                    uint32_t dup = 0;                          // lane bits over which the result is replicated
 #pragma unroll
-                        for (int q = 0; q < PT; ++q) {
-                            part[q].x += __shfl_xor_sync(0xffffffffu, part[q].x, o);
-                            part[q].y += __shfl_xor_sync(0xffffffffu, part[q].y, o);
+                    for (int o = TEAM / 2, width = W0; o >= 1; o >>= 1) {
+                        if (width > 1) {
+                            const int h = width / 2;
+                            const bool hi = (lt & o) != 0;
+#pragma unroll
+                            for (int i = 0; i < W0 / 2; ++i) {
+                                if (i < h) {
+                                    const float keep = hi ? val[i + h] : val[i];
+                                    const float give = hi ? val[i] : val[i + h];
+                                    val[i] = keep + __shfl_xor_sync(0xffffffffu, give, o);
+                                }
+                            }
+                            if (hi) first += h;
+                            width = h;
+                        } else {
+                            val[0] += __shfl_xor_sync(0xffffffffu, val[0], o);
+                            dup |= (uint32_t)o;
                         }
                     }
+                    constexpr int LOGT = TEAM >= 32 ? 5 : TEAM >= 16 ? 4 : TEAM >= 8 ? 3 : TEAM >= 4 ? 2 : TEAM >= 2 ? 1 : 0;
+                    constexpr int WLAST = (W0 >> LOGT) > 1 ? (W0 >> LOGT) : 1;      // floats left per lane
                     const uint32_t code = __float_as_uint(meta.y);
-                    if (ct == 0 && code != 0xffffffffu) {
-                        float2* o = gp.vis_out + (out_base(my_cg) + (long long)(code & 0x7fffffffu)) * P + half * PT;
-                        const float w = (code >> 31) ? 0.f : meta.x;
+                    if ((lt & dup) == 0 && code != 0xffffffffu) {
+                        float* o = reinterpret_cast<float*>(gp.vis_out + (out_base(my_cg) + (long long)(code & 0x7fffffffu)) * P) + first;
+                        const float w = meta.x;
 #pragma unroll
-                        for (int q = 0; q < PT; ++q)
-                            o[q] = (code >> 31) ? make_float2(0.f, 0.f) : make_float2(w * part[q].x, w * part[q].y);
+                        for (int i = 0; i < WLAST; ++i) o[i] = (code >> 31) ? 0.f : w * val[i];
                     }
                     continue;
                 }

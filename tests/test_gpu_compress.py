@@ -87,3 +87,33 @@ def test_compress_edge_cases(oracle_mod):
     assert n_c == 1 and abs(cvis[0, 0] - 5000 * (1.0 + 0.5j)) < 1e-2
     ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, np.full(5000, 2.0, np.float32), kernel)
     assert_parity(grid, ref, "single run")
+
+
+def test_paper_shaped_workload_compressed_full_size(oracle_mod):
+    # 7.26 M samples creeping 0.04 cells per dump (shape of PAPER.md:107-113), compressed on the device and
+    # gridded from the compressed samples, against oracle row bands of the ORIGINAL samples
+    import torch
+    from paper_1605_07023_b200 import binding
+    from gpu_util import REL_L2_TOL, MAX_ABS_TOL
+    cfg = synth.get_config("paper_S16_P1")
+    wl = synth.make_workload(cfg)
+    N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
+    dev = torch.device("cuda:0")
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(cfg.n_vis)
+    plan.allocate_workspace(dev)
+    recs, cvis, n_c = plan.compress(torch.from_numpy(wl.uvw).to(dev), torch.from_numpy(wl.vis).to(dev),
+                                    torch.from_numpy(wl.weights).to(dev))
+    assert cfg.n_vis / n_c > 1.5                                # the regime where compression pays
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+    plan.execute_compressed(recs, cvis, torch.from_numpy(wl.kernel).to(dev), grid)
+    torch.cuda.synchronize()
+    c = N // 2
+    for lo, hi in ((c - 4, c + 4), (c + N // 10, c + N // 10 + 4)):
+        ref = oracle_mod.grid(N, S, O, W, P, wl.uvw, wl.vis, wl.weights, wl.kernel, rows=(lo, hi))
+        got = grid[lo:hi].cpu().numpy().astype(np.complex128)
+        rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+        mx = np.abs(got - ref).max() / np.abs(ref).max()
+        print(f"paper_S16_P1 compressed {cfg.n_vis}->{n_c} rows {lo}:{hi} rel_l2={rel:.2e} max={mx:.2e}")
+        assert rel <= REL_L2_TOL and mx <= MAX_ABS_TOL
+    plan.destroy()

@@ -149,7 +149,7 @@ int grid_plan_set_pol_split(grid_plan* plan, int lanes);
 
 /* HOST out[20]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
  * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, chunk order mode,
- * polarisation split, warp groups per CTA, 0, 0. */
+ * polarisation split, warp groups per CTA, taps in global memory (0/1), 0. */
 int grid_plan_get_info(const grid_plan* plan, int* out);
 
 /* Measurement hook: two caller-owned cudaEvent_t (passed as void*) that the following grid_execute

@@ -83,7 +83,7 @@ def _stream(stream):
 
 
 INFO_FIELDS = ("variant", "cu", "cv", "bin_u", "bin_v", "team_threads", "teams_per_cta",
-               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block", "chunk_order", "pol_split", "groups_per_cta")
+               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block", "chunk_order", "pol_split", "groups_per_cta", "taps_global")
 
 
 class GridPlan:

@@ -47,6 +47,16 @@ __device__ __forceinline__ uint32_t moved_mask(int from, int to) {
     return m & ALL;
 }
 
+// Row-doubled copy of the tap table in global memory (TG kernels): t[r][k] = kern[r][k mod S], k < 2S.
+__global__ void __launch_bounds__(256) tap_table_kernel(const float2* __restrict__ kern, float2* __restrict__ out,
+                                                        long long n_elems, int S) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_elems) return;
+    const long long r = k / (2 * S);
+    const int t = (int)(k - r * 2 * S) & (S - 1);
+    out[k] = __ldg(kern + r * S + t);
+}
+
 struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
     long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)
     int len;                  // mode 0: positions in the chunk; mode 1: channels in the chunk
@@ -97,7 +107,10 @@ struct WarpKernelTraits {
 // registers hold the VALUES of the owned grid points (loaded when the footprint moves onto a new point,
 // where gridding flushes), every sample takes sum conj(G_ij) * value over the owned points, a shuffle
 // tree adds the team's partial sums and one lane stores weight * sum to vis_out.  No atomics.
-template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false>
+// TG: the tap table does not fit shared memory (many w-planes: the paper uses 1229 per slice,
+// PAPER.md:113) -- taps are read through L1/L2 from a row-doubled copy in global memory (gp.gtaps),
+// as the paper's kernel does (Table 1 "unified cache").
+template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false, bool TG = false>
 __global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS, PS>::MAX_THREADS), 1)
 grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
@@ -109,8 +122,8 @@ grid_warp_kernel(const GridParams gp) {
     static_assert(!DEGRID || T::TEAM <= 32, "degridding: a team must fit one warp (shuffle reduction)");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* taps = reinterpret_cast<float2*>(smem_raw);
-    const size_t taps_bytes = ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
+    float2* staps = reinterpret_cast<float2*>(smem_raw);
+    const size_t taps_bytes = TG ? 0 : ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
     const int B = gp.batch, bshift = gp.batch_shift;
     const int slots = TPG * B;
 
@@ -126,9 +139,11 @@ grid_warp_kernel(const GridParams gp) {
     uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
     uint32_t* ctrl = last_pos + 2 * TPG;
 
-    for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {          // a4
-        const int r = k / ROW, t = (k - r * ROW) & (S - 1);
-        taps[k] = __ldg(gp.kern + (size_t)r * S + t);
+    if constexpr (!TG) {
+        for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {      // a4
+            const int r = k / ROW, t = (k - r * ROW) & (S - 1);
+            staps[k] = __ldg(gp.kern + (size_t)r * S + t);
+        }
     }
     __syncthreads();
     if (group >= gp.groups_per_cta) return;            // surplus threads (CTA not a multiple of GT)
@@ -151,8 +166,15 @@ grid_warp_kernel(const GridParams gp) {
     const uint32_t MXY = MX | (MY << 16);              // !WIDE: both masks in one word
     const uint4* my_rec = crec + (size_t)tg * B;
     const float2* my_vis = cvis + (size_t)tg * B * P + (DEGRID ? 0 : half * PT);   // DEGRID: {weight, sample code}
-    const unsigned char* my_tu = reinterpret_cast<const unsigned char*>(taps + r0);
-    const unsigned char* my_tv = reinterpret_cast<const unsigned char*>(taps + s0);
+    const unsigned char* my_tu;
+    const unsigned char* my_tv;
+    if constexpr (TG) {
+        my_tu = reinterpret_cast<const unsigned char*>(gp.gtaps + r0);
+        my_tv = reinterpret_cast<const unsigned char*>(gp.gtaps + s0);
+    } else {
+        my_tu = reinterpret_cast<const unsigned char*>(staps + r0);
+        my_tv = reinterpret_cast<const unsigned char*>(staps + s0);
+    }
     const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
 
     float2 acc[CV][CU][PT];
@@ -366,7 +388,8 @@ grid_warp_kernel(const GridParams gp) {
                 const uint32_t xo = (rec.rows & 0xffffu) * ROW + S - (i0 & (S - 1));
                 const uint32_t yo = (rec.rows >> 16) * ROW + S - (j0 & (S - 1));
                 c.x = rec.pos & 0xffff7fffu;
-                if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
+                if constexpr (WIDE && TG) { c.y = rec.rows; c.z = mx; c.w = my; }     // offsets exceed 16 bits
+                else if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
                 else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
                 valid = (rec.pos & 0x8000u) == 0;
                 if (valid) w = gp.weights ? rw[kk] : 1.f;
@@ -487,7 +510,10 @@ grid_warp_kernel(const GridParams gp) {
                 }
                 const float2* tu;
                 const float2* tv;
-                if constexpr (WIDE) {
+                if constexpr (WIDE && TG) {
+                    tu = reinterpret_cast<const float2*>(my_tu) + (size_t)(c.y & 0xffffu) * ROW + (S - ((c.x & 0x7fffu) & (S - 1)));
+                    tv = reinterpret_cast<const float2*>(my_tv) + (size_t)(c.y >> 16) * ROW + (S - ((c.x >> 16) & (S - 1)));
+                } else if constexpr (WIDE) {
                     tu = reinterpret_cast<const float2*>(my_tu) + (c.y & 0xffffu);
                     tv = reinterpret_cast<const float2*>(my_tv) + (c.y >> 16);
                 } else {

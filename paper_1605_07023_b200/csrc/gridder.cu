@@ -44,6 +44,7 @@ struct grid_plan {
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
     int groups_per_cta, queue_teams;
+    int taps_global;                      // variant 3: tap table read from global memory (too large for shared)
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
     int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on      // variant 3: warp groups per CTA; teams per queue entry (all variants)
@@ -107,6 +108,23 @@ WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps) {
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
+// Kernels that read the taps from global memory (table too large for shared memory): default blocks only.
+template <int CU, int CV, int P>
+WarpDesc pick_tg(int logs) {
+#define TGCASE(l) case l: if constexpr (CU <= (1 << l) && CV <= (1 << l)) { using T = WarpKernelTraits<CU, CV, P, l, 1>; \
+        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; } break;
+    switch (logs) { TGCASE(2) TGCASE(3) TGCASE(4) TGCASE(5) }
+#undef TGCASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+WarpDesc lookup_warp_tg(int cu, int cv, int P, int logs) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_tg<a, b, p>(logs);
+    CASE(2, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1) CASE(2, 2, 2) CASE(4, 2, 2) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
 // Coarsened degridding kernels (grid_warp_kernel<..., DEGRID = true>): teams of at most one warp.
 template <int CU, int CV, int P>
 kernel_fn pick_degrid(int logs) {
@@ -138,6 +156,9 @@ size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 
 // workspace: [256 B counters][order bins][records][chunk order]
 constexpr size_t kHeadBytes = 256 + 2 * kOrderBins * sizeof(uint32_t);
 size_t order_capacity(const grid_plan* p) { return (size_t)(p->n_vis / 8 + 4096); }
+size_t tap_table_bytes(const grid_plan* p) {
+    return p->taps_global ? (size_t)p->W * p->O * 2 * p->S * sizeof(float2) : 0;
+}
 
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
 int derive(grid_plan* p) {
@@ -153,12 +174,25 @@ int derive(grid_plan* p) {
         const int logs = log2_exact(p->S);
         if (logs < 2 || logs > 5)
             return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 32], got %d", p->S);
-        const WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
+        WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
                         p->cu, p->cv, p->pol_split, p->P, p->S);
-        if ((long long)p->W * p->O * 2 * p->S > 65535)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 3: tap table too large for 16-bit offsets");
+        // Tap table: in shared memory when it leaves at least half of it to the warp groups (and, for S = 32,
+        // its offsets fit the record's 16 bits); otherwise read through L1/L2 from global memory (TG kernels).
+        size_t taps = ((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15;
+        p->taps_global = 0;
+        if (taps > (size_t)p->max_smem / 2 || taps + d.group_bytes(p->batch) > (size_t)p->max_smem ||
+            (logs == 5 && (long long)p->W * p->O * 2 * p->S > 65535)) {
+            const WarpDesc g = p->pol_split == 1 ? lookup_warp_tg(p->cu, p->cv, p->P, logs) : WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+            if (!g.fn)
+                return fail(GRID_ERR_UNSUPPORTED, "tap table (%zu B) needs the global-memory kernels, which are instantiated "
+                            "for the default blocks with polarisation split 1 only (got %dx%d, split %d)",
+                            taps, p->cu, p->cv, p->pol_split);
+            d = g;
+            taps = 0;
+            p->taps_global = 1;
+        }
         if (p->batch < 4 || (p->batch & (p->batch - 1)) != 0)
             return fail(GRID_ERR_UNSUPPORTED, "batch %d must be a power of two >= 4", p->batch);
         if (p->chunk < 1) return fail(GRID_ERR_UNSUPPORTED, "chunk %d must be positive", p->chunk);
@@ -174,7 +208,6 @@ int derive(grid_plan* p) {
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
-        const size_t taps = ((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15;
         const size_t per_group = d.group_bytes(p->batch);
         if (taps + per_group > (size_t)p->max_smem)
             return fail(GRID_ERR_UNSUPPORTED, "tap tables (%zu B) + one group's buffers (%zu B) exceed %d B of shared memory",
@@ -278,7 +311,11 @@ void default_tuning(grid_plan* p) {
             trial.batch /= 2;
         }
         if (derive(&trial) == GRID_OK) { *p = trial; return; }
+        // tap table beyond shared memory: the global-memory kernels exist for split 1 and the default blocks
         trial.pol_split = 1;
+        if (trial.P >= 4 && logs == 4) { trial.cu = 4; trial.cv = 2; }
+        trial.batch = 32;
+        if (derive(&trial) == GRID_OK) { *p = trial; return; }
     }
     // a bin must fit one CTA
     while (derive(p) != GRID_OK && p->threads < 512) p->threads *= 2;
@@ -364,7 +401,7 @@ int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_ch
 
 size_t grid_plan_workspace_bytes(const grid_plan* plan) {
     if (!plan || plan->n_vis < 0) return 0;
-    return kHeadBytes + records_bytes(plan) + order_capacity(plan) * sizeof(uint32_t);
+    return kHeadBytes + records_bytes(plan) + ((order_capacity(plan) * sizeof(uint32_t) + 15) & ~(size_t)15) + tap_table_bytes(plan);
 }
 
 int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
@@ -403,7 +440,7 @@ int grid_plan_get_info(const grid_plan* plan, int* out) {
     const int v[20] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
                        plan->teams_per_cta, plan->threads, plan->batch, plan->chunk, plan->ctas_per_sm,
                        plan->smem_bytes, plan->n_sm, plan->traversal, plan->time_block, plan->sort_chunks,
-                       plan->pol_split, plan->groups_per_cta, 0, 0};
+                       plan->pol_split, plan->groups_per_cta, plan->taps_global, 0};
     memcpy(out, v, sizeof(v));
     return GRID_OK;
 }
@@ -571,7 +608,16 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);
+        if (plan->variant == 3 && plan->taps_global) {           // a4: row-doubled table in global memory
+            float2* gt = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes +
+                                                   records_bytes(plan) + ((order_capacity(plan) * sizeof(uint32_t) + 15) & ~(size_t)15));
+            const long long n_elems = (long long)plan->W * plan->O * 2 * plan->S;
+            tap_table_kernel<<<(unsigned)((n_elems + 255) / 256), 256, 0, stream>>>(gp.kern, gt, n_elems, plan->S);
+            gp.gtaps = gt;
+            plan->last_launches++;
+        }
         kernel_fn fn = degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs)
+                     : (plan->variant == 3 && plan->taps_global) ? lookup_warp_tg(plan->cu, plan->cv, plan->P, logs).fn
                      : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
@@ -679,7 +725,7 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
     if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
         return fail(GRID_ERR_STATE, "grid_degrid: workspace missing or smaller than grid_plan_workspace_bytes()");
     // the coarsened, register-resident kernel where the plan offers one; the gather kernel otherwise
-    if (plan->variant == 3 && plan->degrid_gather == 0) {
+    if (plan->variant == 3 && plan->degrid_gather == 0 && !plan->taps_global) {
         grid_plan tmp = *plan;                       // same plan with polarisation split 1 (shuffle reduction per team)
         tmp.pol_split = 1;
         tmp.threads = 1024;

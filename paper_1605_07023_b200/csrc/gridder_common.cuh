@@ -36,6 +36,7 @@ struct GridParams {
     const float2* vis;        // [n_vis][P]
     const float* weights;     // [n_vis]
     const float2* kern;       // [W][O][S]
+    const float2* gtaps;      // variant 3, tap table too large for shared memory: rows doubled, in global memory
     float* grid;              // [N][N][P] complex64
     float2* vis_out;          // degridding only: [n_vis][P] complex64 result
     unsigned int* counters;   // [0]: next chunk group

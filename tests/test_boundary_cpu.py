@@ -65,7 +65,7 @@ def test_workspace_and_tuning(binding):
     assert plan.workspace_bytes() == 0              # set_samples not called yet
     plan.set_samples(1001)
     head = 256 + 2 * 1024 * 4                       # counters + chunk-order bins
-    assert plan.workspace_bytes() == head + 1004 * 16 + (1001 // 8 + 4096) * 4
+    assert plan.workspace_bytes() == head + 1004 * 16 + ((1001 // 8 + 4096) * 4 + 15) // 16 * 16
     plan.set_samples(0)
     assert plan.workspace_bytes() == head + 4096 * 4
     plan.set_layout(10, 10, 10)

@@ -194,6 +194,19 @@ def test_sorted_chunk_queue(oracle_mod, name, ps, mode):
     assert_parity(got, ref, f"{name} sorted queue mode={mode}")
 
 
+@pytest.mark.parametrize("S,W,P", [(16, 700, 1), (32, 300, 4), (8, 1500, 4), (32, 1229, 1), (4, 4000, 1), (16, 520, 2)])
+def test_tap_table_beyond_shared_memory(oracle_mod, S, W, P):
+    # many w-planes (the paper: 1229 per slice): the plan switches to the kernels that read the
+    # taps from global memory; same result as the oracle, also through the compressed entry point
+    N, O, n = 192, 8, 25_001
+    uvw, vis, wts, kernel = synth.random_problem(500 + S + P, n, N, S, O, W, P, spread=0.5, walk=0.7)
+    assert len(np.unique(np.floor(uvw[:, 2]))) > 0.2 * min(W, n)             # planes all over the table
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel)
+    assert info["variant"] == 3 and info["taps_global"] == 1 and info["launches"] == 3
+    assert_parity(got, ref, f"global taps S={S} W={W} P={P} {info}")
+
+
 def test_inconsistent_layout_hint_is_ignored(oracle_mod):
     cfg = synth.shrink(synth.get_config("cfg1"), n_ant=8, n_times=16, n_chan=8, grid_size=256)
     wl = synth.make_workload(cfg)

@@ -67,12 +67,13 @@ CONFIGS = {
 }
 
 
-def paper_regime_config(support: int, n_pol: int) -> Config:
+def paper_regime_config(support: int, n_pol: int, n_wplanes: int = 16) -> Config:
     """Shape of the paper's own workload: 64 antennas, one channel, 2 h of 2-s dumps =
     2016 x 3600 = 7 257 600 samples that move a fraction of a cell per dump.  Synthetic antennas and
     visibilities as everywhere else; NOT the paper's data set.  Context measurement only."""
-    return Config(f"paper_S{support}_P{n_pol}", 7, 64, "disk", 4000.0, 3600, 2.0, 1, 1.4e9, 1.4e9, n_pol, 4096,
-                  support, 8, 16, "kb_chirp", False)
+    name = f"paper_S{support}_P{n_pol}" + ("" if n_wplanes == 16 else f"_W{n_wplanes}")
+    return Config(name, 7, 64, "disk", 4000.0, 3600, 2.0, 1, 1.4e9, 1.4e9, n_pol, 4096,
+                  support, 8, n_wplanes, "kb_chirp", False)
 
 
 def sweep_config(support: int, n_pol: int) -> Config:
@@ -86,8 +87,9 @@ def get_config(name: str) -> Config:
     if name in CONFIGS:
         return CONFIGS[name]
     if name.startswith("paper_S"):
-        s, p = name[len("paper_S"):].split("_P")
-        return paper_regime_config(int(s), int(p))
+        s, rest = name[len("paper_S"):].split("_P")
+        p, _, w = rest.partition("_W")
+        return paper_regime_config(int(s), int(p), int(w) if w else 16)
     if name.startswith("cfg4_S"):
         s, p = name[len("cfg4_S"):].split("_P")
         return sweep_config(int(s), int(p))

@@ -107,3 +107,45 @@ def test_full_size_degrid_sampled(oracle_mod, name):
     # every output was written: no sample left at the allocation's garbage (finite everywhere, right count of zeros)
     assert bool(torch.isfinite(torch.view_as_real(out)).all())
     plan.destroy()
+
+
+@pytest.mark.parametrize("N,P,S", [(32767, 1, 8), (16001, 4, 16)])
+def test_maximum_grid_size_corners(oracle_mod, N, P, S):
+    # the largest grid the ABI accepts (N = 32767, odd: rows are not 16-byte aligned) and an odd 4-pol one
+    # beyond 2^31 bytes: samples in the four corners, on the last valid cell, and in the centre -- 32/64-bit
+    # index arithmetic of the flush addresses.  The oracle computes the touched row bands only.
+    import torch
+    from paper_1605_07023_b200 import binding
+    O, W = 4, 2
+    rng = np.random.default_rng(N)
+    half = N // 2
+    lo_u, hi_u = -half + S / 2.0, N - 1 - half - S / 2.0 + 0.4          # first / last footprint that still fits
+    corners = [(lo_u, lo_u), (lo_u, hi_u), (hi_u, lo_u), (hi_u, hi_u), (0.3, -0.2), (hi_u + 1.0, 0.0)]   # last one: off grid
+    uv = np.repeat(np.array(corners, dtype=np.float64), 40, axis=0) + rng.uniform(-0.4, 0.0, (40 * len(corners), 2))
+    n = len(uv)
+    uvw = np.concatenate([uv, rng.uniform(0, W, (n, 1))], axis=1).astype(np.float32)
+    vis = (rng.standard_normal((n, P)) + 1j * rng.standard_normal((n, P))).astype(np.complex64)
+    wts = rng.uniform(0.5, 1, n).astype(np.float32)
+    kernel = (rng.standard_normal((W, O, S)) + 1j * rng.standard_normal((W, O, S))).astype(np.complex64)
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    assert q["valid"][:200].all() and not q["valid"][200:].any()
+    assert q["i0"][:200].min() == 0 and (q["i0"][:200] + S).max() == N and (q["j0"][:200] + S).max() == N
+    dev = torch.device("cuda:0")
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(n)
+    plan.allocate_workspace(dev)
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+    plan.execute(torch.from_numpy(uvw).to(dev), torch.from_numpy(vis).to(dev), torch.from_numpy(wts).to(dev),
+                 torch.from_numpy(kernel).to(dev), grid)
+    torch.cuda.synchronize()
+    touched = 0
+    for lo, hi in ((0, 2 * S), (half - 2 * S, half + 2 * S), (N - 2 * S, N)):
+        ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel, rows=(lo, hi))
+        got = grid[lo:hi].cpu().numpy().astype(np.complex128)
+        assert np.abs(ref).max() > 0
+        assert np.linalg.norm(got - ref) <= REL_L2_TOL * np.linalg.norm(ref)
+        assert np.abs(got - ref).max() <= MAX_ABS_TOL * np.abs(ref).max()
+        touched += int((got != 0).sum())
+    # nothing landed anywhere else
+    assert int((torch.view_as_real(grid) != 0).any(dim=-1).sum().item()) == touched
+    plan.destroy()

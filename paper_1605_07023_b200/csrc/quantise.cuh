@@ -99,6 +99,15 @@ quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, lon
     } else {
         for (int k = 0; k < 12; ++k) c[k] = (first * 3 + k < n * 3) ? __ldg(uvw + first * 3 + k) : 0.f;
     }
+    if (qp.format == 1 && first + 4 <= n) {          // four 8-byte records = two 16-byte stores
+        CycRec r[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) r[k] = make_cyc_record(quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp), qp);
+        uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<CycRec*>(recs) + first);
+        dst[0] = make_uint4(r[0].pos, r[0].rows, r[1].pos, r[1].rows);
+        dst[1] = make_uint4(r[2].pos, r[2].rows, r[3].pos, r[3].rows);
+        return;
+    }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         if (first + k < n) {

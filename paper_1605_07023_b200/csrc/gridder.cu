@@ -319,6 +319,14 @@ void default_tuning(grid_plan* p) {
     }
     // a bin must fit one CTA
     while (derive(p) != GRID_OK && p->threads < 512) p->threads *= 2;
+    if (derive(p) != GRID_OK) {
+        // supports whose bin exceeds a CTA (tiles across CTAs, are not built): smaller blocks,
+        // and as the last resort the one-atomic-per-update kernel, which handles any support
+        const int tries[4][2] = {{4, 2}, {2, 2}, {2, 1}, {1, 1}};
+        for (int t = 0; t < 4 && derive(p) != GRID_OK; ++t) { p->cu = tries[t][0]; p->cv = tries[t][1]; p->threads = 512; }
+        if (derive(p) != GRID_OK) { p->variant = 0; p->cu = p->cv = 1; }
+        g_err[0] = 0;
+    }
 }
 
 long long ctas_hint(const grid_plan* p) { return (long long)p->n_sm * (p->groups_per_cta > 0 ? p->groups_per_cta : 1); }

@@ -217,6 +217,18 @@ def test_inconsistent_layout_hint_is_ignored(oracle_mod):
     assert_parity(got, ref, "bad layout")
 
 
+@pytest.mark.parametrize("S,P", [(64, 4), (128, 1), (100, 2), (48, 4)])
+def test_large_supports_have_a_path(oracle_mod, S, P):
+    # the ABI accepts supports up to 128 (the paper's bins: 32, 64, 128): whatever kernel the plan falls back
+    # to (smaller blocks, or one atomic per update when a bin exceeds a CTA), the result is the oracle's
+    N, O, W, n = 512, 2, 2, 3_001
+    uvw, vis, wts, kernel = synth.random_problem(900 + S + P, n, N, S, O, W, P, spread=0.45, walk=0.5)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel)
+    print(S, P, info)
+    assert_parity(got, ref, f"S={S} P={P} {info}")
+
+
 def test_scatter_variant(oracle_mod):
     N, S, O, W, P, n = 128, 6, 4, 2, 4, 5001
     uvw, vis, wts, kernel = synth.random_problem(42, n, N, S, O, W, P, spread=0.52)

@@ -24,6 +24,7 @@
 //     memory by the group's own lanes (pre-weighting PAPER.md:91, tap offsets, moved masks) while the
 //     next batch is in flight.
 #pragma once
+#include <type_traits>
 #include "gridder_common.cuh"
 #include "grid_kernel.cuh"             // red_add_v2 / red_add_v4
 #include "chunk_order.cuh"
@@ -55,6 +56,19 @@ __global__ void __launch_bounds__(256) tap_table_kernel(const float2* __restrict
     const long long r = k / (2 * S);
     const int t = (int)(k - r * 2 * S) & (S - 1);
     out[k] = __ldg(kern + r * S + t);
+}
+
+// The same for a 64-wide bin (S = 64): 64-bit mask.
+__device__ __forceinline__ uint64_t moved_mask64(int from, int to) {
+    const int d = to - from;
+    if (d == 0) return 0ull;
+    const int ad = d < 0 ? -d : d;
+    if (ad >= 64) return ~0ull;
+    const int start = (d > 0 ? from : to) & 63;
+    const uint64_t run = (1ull << ad) - 1ull;
+    uint64_t m = run << start;
+    if (start) m |= run >> (64 - start);
+    return m;
 }
 
 struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
@@ -95,7 +109,8 @@ struct WarpKernelTraits {
     static constexpr int ACC = 2 * CU * CV * PT;
     static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
     // shared memory of one group for a batch of B samples per team
-    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + 8 * P); }
+    static constexpr bool W64 = LOGS == 6;                // 64-bit moved masks live in a second 16-byte record
+    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + (W64 ? 16 : 0) + 8 * P); }
     __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
     __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
     __host__ __device__ static constexpr size_t group_bytes(int B) {
@@ -117,7 +132,9 @@ grid_warp_kernel(const GridParams gp) {
     constexpr int PT = T::PT;
     constexpr int S = T::S, DU = T::DU, DV = T::DV, TEAM = T::TEAM, GW = T::GW, GT = T::GT, TPG = T::TPG;
     constexpr int ROW = 2 * S;                         // doubled tap row k[t mod S], t < 2S: offsets reach 2S-1
-    constexpr bool WIDE = S > 16;                      // record format: 32-bit masks need two words
+    constexpr bool W64 = T::W64;                       // S = 64: {pos, tap rows, -, -} + a mask record {mx, my} of 64 bits each
+    constexpr bool WIDE = S == 32;                     // record format: 32-bit masks need two words
+    using mask_t = typename std::conditional<W64, uint64_t, uint32_t>::type;
     static_assert(CU <= S && CV <= S, "block larger than the support");
     static_assert(!DEGRID || T::TEAM <= 32, "degridding: a team must fit one warp (shuffle reduction)");
 
@@ -132,6 +149,7 @@ grid_warp_kernel(const GridParams gp) {
     unsigned char* gbase = smem_raw + taps_bytes + (size_t)group * T::group_bytes(B);
     uint4* crec = reinterpret_cast<uint4*>(gbase);                                       // cooked records
     float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)slots * 16);                // cooked vis
+    uint4* cmask = reinterpret_cast<uint4*>(gbase + (size_t)slots * (16 + 8 * P));       // W64 only
     unsigned char* rbase = gbase + T::cooked_bytes(B);
     const size_t rstage = T::raw_bytes(B);
     // raw stage layout: vis [slots][P] float2, rec [slots] 8 B, weights [slots] float
@@ -158,12 +176,13 @@ grid_warp_kernel(const GridParams gp) {
     const int lt = lg - tg * TEAM;
     const int half = lt % PS, ct = lt / PS;            // my share of the polarisations; my block owner index
     const int r0 = ct % DU, s0 = ct / DU;
-    uint32_t MX = 0, MY = 0;
+    mask_t MX = 0, MY = 0;
 #pragma unroll
-    for (int a = 0; a < CU; ++a) MX |= 1u << (r0 + a * DU);
+    for (int a = 0; a < CU; ++a) MX |= mask_t(1) << (r0 + a * DU);
 #pragma unroll
-    for (int b = 0; b < CV; ++b) MY |= 1u << (s0 + b * DV);
-    const uint32_t MXY = MX | (MY << 16);              // !WIDE: both masks in one word
+    for (int b = 0; b < CV; ++b) MY |= mask_t(1) << (s0 + b * DV);
+    const uint32_t MXY = (uint32_t)MX | ((uint32_t)MY << 16);      // S <= 16: both masks in one word
+    const uint4* my_mask = cmask + (size_t)tg * B;
     const uint4* my_rec = crec + (size_t)tg * B;
     const float2* my_vis = cvis + (size_t)tg * B * P + (DEGRID ? 0 : half * PT);   // DEGRID: {weight, sample code}
     const unsigned char* my_tu;
@@ -375,20 +394,30 @@ grid_warp_kernel(const GridParams gp) {
             uint4 c = make_uint4(0u, 0u, 0u, 0u);
             float w = 0.f;
             bool valid = false;
+            if constexpr (W64) cmask[kk] = make_uint4(0u, 0u, 0u, 0u);
             if (k < cnt) {
                 const CycRec rec = rrec[kk];
-                uint32_t mx = 0, my = 0;
+                mask_t mx = 0, my = 0;
                 if (k > 0 || b > 0) {
                     const uint32_t pp = k > 0 ? rrec[kk - 1].pos : last_pos[((b - 1) & 1) * TPG + t];
-                    mx = moved_mask<LOGS>((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
-                    my = moved_mask<LOGS>((int)(pp >> 16), (int)(rec.pos >> 16));
+                    if constexpr (W64) {
+                        mx = moved_mask64((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
+                        my = moved_mask64((int)(pp >> 16), (int)(rec.pos >> 16));
+                    } else {
+                        mx = moved_mask<LOGS>((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
+                        my = moved_mask<LOGS>((int)(pp >> 16), (int)(rec.pos >> 16));
+                    }
                 }
                 if (k == cnt - 1) last_pos[(b & 1) * TPG + t] = rec.pos;
                 const int i0 = (int)(rec.pos & 0x7fffu), j0 = (int)(rec.pos >> 16);
                 const uint32_t xo = (rec.rows & 0xffffu) * ROW + S - (i0 & (S - 1));
                 const uint32_t yo = (rec.rows >> 16) * ROW + S - (j0 & (S - 1));
                 c.x = rec.pos & 0xffff7fffu;
-                if constexpr (WIDE && TG) { c.y = rec.rows; c.z = mx; c.w = my; }     // offsets exceed 16 bits
+                if constexpr (W64) {
+                    c.y = rec.rows;
+                    cmask[kk] = make_uint4((uint32_t)mx, (uint32_t)((uint64_t)mx >> 32), (uint32_t)my, (uint32_t)((uint64_t)my >> 32));
+                }
+                else if constexpr (WIDE && TG) { c.y = rec.rows; c.z = mx; c.w = my; }     // offsets exceed 16 bits
                 else if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
                 else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
                 valid = (rec.pos & 0x8000u) == 0;
@@ -459,31 +488,42 @@ grid_warp_kernel(const GridParams gp) {
                 const uint4 c = c_next;
                 c_next = *++rp;                        // next record (one slot of slack follows the batch)
                 bool moved;
-                if constexpr (WIDE) moved = ((c.z & MX) | (c.w & MY)) != 0;
-                else moved = (c.w & MXY) != 0;
+                mask_t mx_all = 0, my_all = 0;             // this sample's moved masks
+                if constexpr (W64) {
+                    const uint4 m = my_mask[s];
+                    mx_all = (uint64_t)m.x | ((uint64_t)m.y << 32);
+                    my_all = (uint64_t)m.z | ((uint64_t)m.w << 32);
+                    moved = ((mx_all & MX) | (my_all & MY)) != 0;
+                } else if constexpr (WIDE) {
+                    mx_all = c.z; my_all = c.w;
+                    moved = ((c.z & MX) | (c.w & MY)) != 0;
+                } else {
+                    mx_all = c.w; my_all = c.w >> 16;
+                    moved = (c.w & MXY) != 0;
+                }
                 if (moved) {                           // a5/a8: some of my points moved
                     const int i0 = (int)(c.x & 0x7fffu), j0 = (int)(c.x >> 16);
-                    const uint32_t mxs = (WIDE ? c.z : c.w) >> r0;
-                    const uint32_t mys = (WIDE ? c.w : (c.w >> 16)) >> s0;
+                    const mask_t mxs = mx_all >> r0;
+                    const mask_t mys = my_all >> s0;
                     if constexpr (DEGRID) {
                         // positions first, then the values of every point that changed (a point whose
                         // column AND row moved is fetched twice; harmless)
 #pragma unroll
                         for (int a = 0; a < CU; ++a)
-                            if (mxs & (1u << (a * DU))) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+                            if (mxs & (mask_t(1) << (a * DU))) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
 #pragma unroll
                         for (int bb = 0; bb < CV; ++bb)
-                            if (mys & (1u << (bb * DV))) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                            if (mys & (mask_t(1) << (bb * DV))) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
 #pragma unroll
                         for (int a = 0; a < CU; ++a) {
-                            if (mxs & (1u << (a * DU))) {
+                            if (mxs & (mask_t(1) << (a * DU))) {
 #pragma unroll
                                 for (int bb = 0; bb < CV; ++bb) load_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
                             }
                         }
 #pragma unroll
                         for (int bb = 0; bb < CV; ++bb) {
-                            if (mys & (1u << (bb * DV))) {
+                            if (mys & (mask_t(1) << (bb * DV))) {
 #pragma unroll
                                 for (int a = 0; a < CU; ++a) load_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
                             }
@@ -491,7 +531,7 @@ grid_warp_kernel(const GridParams gp) {
                     } else {
 #pragma unroll
                     for (int a = 0; a < CU; ++a) {
-                        if (mxs & (1u << (a * DU))) {  // owned column a left the footprint
+                        if (mxs & (mask_t(1) << (a * DU))) {  // owned column a left the footprint
 #pragma unroll
                             for (int bb = 0; bb < CV; ++bb) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
                             cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
@@ -499,10 +539,10 @@ grid_warp_kernel(const GridParams gp) {
                     }
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb) {
-                        if (mys & (1u << (bb * DV))) { // owned row bb left the footprint
+                        if (mys & (mask_t(1) << (bb * DV))) { // owned row bb left the footprint
 #pragma unroll
                             for (int a = 0; a < CU; ++a)
-                                flush_point_if(acc[bb][a], ry[bb] + (uint32_t)cx[a], mxs & (1u << (a * DU)));
+                                flush_point_if(acc[bb][a], ry[bb] + (uint32_t)cx[a], (mxs & (mask_t(1) << (a * DU))) ? 1u : 0u);
                             ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
                         }
                     }
@@ -510,7 +550,7 @@ grid_warp_kernel(const GridParams gp) {
                 }
                 const float2* tu;
                 const float2* tv;
-                if constexpr (WIDE && TG) {
+                if constexpr (W64 || (WIDE && TG)) {
                     tu = reinterpret_cast<const float2*>(my_tu) + (size_t)(c.y & 0xffffu) * ROW + (S - ((c.x & 0x7fffu) & (S - 1)));
                     tv = reinterpret_cast<const float2*>(my_tv) + (size_t)(c.y >> 16) * ROW + (S - ((c.x >> 16) & (S - 1)));
                 } else if constexpr (WIDE) {

@@ -94,6 +94,7 @@ WarpDesc pick_warp(int logs) {
         case 3: return WarpPick<CU, CV, P, 3, PS>::get();
         case 4: return WarpPick<CU, CV, P, 4, PS>::get();
         case 5: return WarpPick<CU, CV, P, 5, PS>::get();
+        case 6: if constexpr (PS == 1 && CU * CV >= 4) return WarpPick<CU, CV, P, 6, PS>::get(); break;   // teams <= 1024 threads
     }
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -111,9 +112,14 @@ WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps) {
 // Kernels that read the taps from global memory (table too large for shared memory): default blocks only.
 template <int CU, int CV, int P>
 WarpDesc pick_tg(int logs) {
-#define TGCASE(l) case l: if constexpr (CU <= (1 << l) && CV <= (1 << l)) { using T = WarpKernelTraits<CU, CV, P, l, 1>; \
-        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; } break;
-    switch (logs) { TGCASE(2) TGCASE(3) TGCASE(4) TGCASE(5) }
+#define TGBODY(l) if constexpr (CU <= (1 << l) && CV <= (1 << l)) { using T = WarpKernelTraits<CU, CV, P, l, 1>; \
+        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; }
+#define TGCASE(l) case l: TGBODY(l) break;
+    switch (logs) {
+        TGCASE(2) TGCASE(3) TGCASE(4) TGCASE(5)
+        case 6: if constexpr (CU * CV >= 4) { TGBODY(6) } break;
+    }
+#undef TGBODY
 #undef TGCASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -172,8 +178,8 @@ int derive(grid_plan* p) {
     p->groups_per_cta = 0;
     if (p->variant == 3) {
         const int logs = log2_exact(p->S);
-        if (logs < 2 || logs > 5)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 32], got %d", p->S);
+        if (logs < 2 || logs > 6)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 64], got %d", p->S);
         WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
@@ -283,7 +289,7 @@ void default_tuning(grid_plan* p) {
     if (p->S < 4) { p->cu = 1; p->cv = 1; }
     // power-of-two supports: bin == support, no padding (grid_warp_kernel.cuh)
     const int logs = log2_exact(p->S);
-    if (logs >= 2 && logs <= 5) {
+    if (logs >= 2 && logs <= 6) {
         grid_plan trial = *p;
         trial.variant = 3;
         trial.threads = 1024;              // clipped to the kernel's register-limited maximum
@@ -298,9 +304,9 @@ void default_tuning(grid_plan* p) {
             else if (logs == 4) { trial.cu = 4; trial.cv = 4; trial.pol_split = 2; }
             else { trial.cu = 4; trial.cv = 2; trial.pol_split = 1; }
         }
-        else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = 2; }
+        else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = (logs == 6) ? 4 : 2; }
         else if (logs == 2) { trial.cu = 2; trial.cv = 2; }
-        else if (logs == 5) { trial.cu = 8; trial.cv = 4; }
+        else if (logs >= 5) { trial.cu = 8; trial.cv = 4; }
         else { trial.cu = 4; trial.cv = 4; }
         // several teams share a warp at small supports: shrink the batch until all warps fit
         while (trial.batch > 8) {

@@ -113,7 +113,7 @@ int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid
 
 /* Override the tuned launch configuration (autotuning).  Any argument <= 0 keeps the
  * current value.  variant: 3 = warp-autonomous coarsened kernel with bin == support (power-of-two
- * supports 4..64; default for those), 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any
+ * supports 4..128; default for those), 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any
  * support; default otherwise), 0 = naive scatter (one atomic per update; diagnostic baseline only).
  *   cu, cv            coarsening block per thread (u, v), each in {1,2,4,8}, cu*cv*n_pol <= 32
  *   threads_per_cta   multiple of 32, <= 1024

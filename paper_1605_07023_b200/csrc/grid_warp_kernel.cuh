@@ -71,13 +71,28 @@ __device__ __forceinline__ uint64_t moved_mask64(int from, int to) {
     return m;
 }
 
+// S = 128 is split into 2 x 2 tiles of 64 x 64 bin positions, one team per tile ("one
+// work-group per tile"; every tile reads the chunk's samples again).  Moved positions of the 64-wide
+// window starting at bin position `lo`.
+__device__ __forceinline__ uint64_t moved_mask_window128(int from, int to, int lo) {
+    const int d = to - from;
+    if (d == 0) return 0ull;
+    const int ad = d < 0 ? -d : d;
+    if (ad >= 128) return ~0ull;
+    const int rel = (((d > 0 ? from : to) - lo) & 127);          // run [rel, rel + ad) in window coordinates, cyclic mod 128
+    const unsigned __int128 run = (((unsigned __int128)1) << ad) - 1;
+    unsigned __int128 m = run << rel;
+    if (rel) m |= run >> (128 - rel);
+    return (uint64_t)m;
+}
+
 struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
     long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)
     int len;                  // mode 0: positions in the chunk; mode 1: channels in the chunk
     int h;                    // mode 1: time steps in this block (0: empty chunk)
     int col0, rowpar;         // mode 0 with layout: column of `base` and parity of its time row;
                               // mode 1: first channel of the chunk
-    int pad0, pad1;
+    int tile, pad1;           // S = 128: which 64 x 64 tile of the bin this team covers (x + 2 y)
 };
 
 __device__ __forceinline__ void cp_async_4(void* dst, const void* src) {
@@ -101,15 +116,17 @@ struct WarpKernelTraits {
     static_assert(P % PS == 0, "polarisations must divide evenly over the split");
     static constexpr int S = 1 << LOGS;
     static constexpr int PT = P / PS;                     // polarisations per thread
-    static constexpr int DU = S / CU, DV = S / CV;       // spacing of a thread's owned positions
-    static constexpr int TEAM = DU * DV * PS;             // threads per bin
+    static constexpr int TS = S > 64 ? 64 : S;            // side of the part of the bin one team covers (tile)
+    static constexpr int NT = (S / TS) * (S / TS);        // tiles per bin (1, or 4 at S = 128)
+    static constexpr int DU = TS / CU, DV = TS / CV;     // spacing of a thread's owned positions
+    static constexpr int TEAM = DU * DV * PS;             // threads per tile
     static constexpr int GW = TEAM > 32 ? TEAM / 32 : 1;  // warps per group
     static constexpr int GT = GW * 32;                    // threads per group
     static constexpr int TPG = TEAM >= 32 ? 1 : 32 / TEAM;    // teams (chunks in flight) per group
     static constexpr int ACC = 2 * CU * CV * PT;
     static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
     // shared memory of one group for a batch of B samples per team
-    static constexpr bool W64 = LOGS == 6;                // 64-bit moved masks live in a second 16-byte record
+    static constexpr bool W64 = TS == 64;                 // 64-bit moved masks live in a second 16-byte record
     __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + (W64 ? 16 : 0) + 8 * P); }
     __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
     __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
@@ -131,11 +148,13 @@ grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
     constexpr int PT = T::PT;
     constexpr int S = T::S, DU = T::DU, DV = T::DV, TEAM = T::TEAM, GW = T::GW, GT = T::GT, TPG = T::TPG;
+    constexpr int TS = T::TS, NT = T::NT;
+    static_assert(NT == 1 || TPG == 1, "tiled bins: one team per group");
     constexpr int ROW = 2 * S;                         // doubled tap row k[t mod S], t < 2S: offsets reach 2S-1
     constexpr bool W64 = T::W64;                       // S = 64: {pos, tap rows, -, -} + a mask record {mx, my} of 64 bits each
     constexpr bool WIDE = S == 32;                     // record format: 32-bit masks need two words
     using mask_t = typename std::conditional<W64, uint64_t, uint32_t>::type;
-    static_assert(CU <= S && CV <= S, "block larger than the support");
+    static_assert(CU <= TS && CV <= TS, "block larger than the support");
     static_assert(!DEGRID || T::TEAM <= 32, "degridding: a team must fit one warp (shuffle reduction)");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -291,14 +310,14 @@ grid_warp_kernel(const GridParams gp) {
         }
         const long long g = v;
         if (g < n_groups && lg < TPG) {
-            long long chunk_id = g * TPG + lg;
+            long long chunk_id = (g / NT) * TPG + lg;      // tiled bins: NT consecutive queue entries share a chunk
             bool have = true;
             if (gp.order) {                            // locality-sorted queue (chunk_order.cuh)
                 have = chunk_id < chunk_count(gp, mode);
                 if (have) chunk_id = __ldg(gp.order + chunk_id);
             }
             WarpChunk cg;
-            cg.base = 0; cg.len = 0; cg.h = 0; cg.col0 = 0; cg.rowpar = 0; cg.pad0 = cg.pad1 = 0;
+            cg.base = 0; cg.len = 0; cg.h = 0; cg.col0 = 0; cg.rowpar = 0; cg.tile = (int)(g % NT); cg.pad1 = 0;
             if (!have) {
             } else if (mode == 0) {
                 cg.base = chunk_id * gp.chunk;
@@ -400,7 +419,10 @@ grid_warp_kernel(const GridParams gp) {
                 mask_t mx = 0, my = 0;
                 if (k > 0 || b > 0) {
                     const uint32_t pp = k > 0 ? rrec[kk - 1].pos : last_pos[((b - 1) & 1) * TPG + t];
-                    if constexpr (W64) {
+                    if constexpr (NT > 1) {
+                        mx = moved_mask_window128((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu), (cg.tile & 1) * TS);
+                        my = moved_mask_window128((int)(pp >> 16), (int)(rec.pos >> 16), (cg.tile >> 1) * TS);
+                    } else if constexpr (W64) {
                         mx = moved_mask64((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
                         my = moved_mask64((int)(pp >> 16), (int)(rec.pos >> 16));
                     } else {
@@ -446,6 +468,8 @@ grid_warp_kernel(const GridParams gp) {
     int st = 0;                                        // raw stage holding the next batch to cook
     while (cur < n_groups) {
         const WarpChunk my_cg = geom[par * TPG + tg];
+        // first owned column / row position (inside my tile of the bin when the bin is tiled)
+        const int px0 = r0 + (NT > 1 ? (my_cg.tile & 1) * TS : 0), py0 = s0 + (NT > 1 ? (my_cg.tile >> 1) * TS : 0);
         bool live = false;
         long long next = cur;
         int next_par = par;
@@ -469,9 +493,9 @@ grid_warp_kernel(const GridParams gp) {
                 const uint32_t p0 = my_rec[0].x;
                 const int i0 = (int)(p0 & 0x7fffu), j0 = (int)(p0 >> 16);
 #pragma unroll
-                for (int a = 0; a < CU; ++a) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+                for (int a = 0; a < CU; ++a) cx[a] = i0 + ((px0 + a * DU - i0) & (S - 1));
 #pragma unroll
-                for (int bb = 0; bb < CV; ++bb) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                for (int bb = 0; bb < CV; ++bb) ry[bb] = (uint32_t)(j0 + ((py0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
                 if constexpr (DEGRID) {
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb)
@@ -510,10 +534,10 @@ grid_warp_kernel(const GridParams gp) {
                         // column AND row moved is fetched twice; harmless)
 #pragma unroll
                         for (int a = 0; a < CU; ++a)
-                            if (mxs & (mask_t(1) << (a * DU))) cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+                            if (mxs & (mask_t(1) << (a * DU))) cx[a] = i0 + ((px0 + a * DU - i0) & (S - 1));
 #pragma unroll
                         for (int bb = 0; bb < CV; ++bb)
-                            if (mys & (mask_t(1) << (bb * DV))) ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                            if (mys & (mask_t(1) << (bb * DV))) ry[bb] = (uint32_t)(j0 + ((py0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
 #pragma unroll
                         for (int a = 0; a < CU; ++a) {
                             if (mxs & (mask_t(1) << (a * DU))) {
@@ -534,7 +558,7 @@ grid_warp_kernel(const GridParams gp) {
                         if (mxs & (mask_t(1) << (a * DU))) {  // owned column a left the footprint
 #pragma unroll
                             for (int bb = 0; bb < CV; ++bb) flush_point(acc[bb][a], ry[bb] + (uint32_t)cx[a]);
-                            cx[a] = i0 + ((r0 + a * DU - i0) & (S - 1));
+                            cx[a] = i0 + ((px0 + a * DU - i0) & (S - 1));
                         }
                     }
 #pragma unroll
@@ -543,7 +567,7 @@ grid_warp_kernel(const GridParams gp) {
 #pragma unroll
                             for (int a = 0; a < CU; ++a)
                                 flush_point_if(acc[bb][a], ry[bb] + (uint32_t)cx[a], (mxs & (mask_t(1) << (a * DU))) ? 1u : 0u);
-                            ry[bb] = (uint32_t)(j0 + ((s0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
+                            ry[bb] = (uint32_t)(j0 + ((py0 + bb * DV - j0) & (S - 1))) * (uint32_t)gp.N;
                         }
                     }
                     }
@@ -551,8 +575,8 @@ grid_warp_kernel(const GridParams gp) {
                 const float2* tu;
                 const float2* tv;
                 if constexpr (W64 || (WIDE && TG)) {
-                    tu = reinterpret_cast<const float2*>(my_tu) + (size_t)(c.y & 0xffffu) * ROW + (S - ((c.x & 0x7fffu) & (S - 1)));
-                    tv = reinterpret_cast<const float2*>(my_tv) + (size_t)(c.y >> 16) * ROW + (S - ((c.x >> 16) & (S - 1)));
+                    tu = reinterpret_cast<const float2*>(my_tu) + (size_t)(c.y & 0xffffu) * ROW + (S - ((c.x & 0x7fffu) & (S - 1))) + (px0 - r0);
+                    tv = reinterpret_cast<const float2*>(my_tv) + (size_t)(c.y >> 16) * ROW + (S - ((c.x >> 16) & (S - 1))) + (py0 - s0);
                 } else if constexpr (WIDE) {
                     tu = reinterpret_cast<const float2*>(my_tu) + (c.y & 0xffffu);
                     tv = reinterpret_cast<const float2*>(my_tv) + (c.y >> 16);

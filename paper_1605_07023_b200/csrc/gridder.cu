@@ -95,6 +95,7 @@ WarpDesc pick_warp(int logs) {
         case 4: return WarpPick<CU, CV, P, 4, PS>::get();
         case 5: return WarpPick<CU, CV, P, 5, PS>::get();
         case 6: if constexpr (PS == 1 && CU * CV >= 4) return WarpPick<CU, CV, P, 6, PS>::get(); break;   // teams <= 1024 threads
+        case 7: if constexpr (PS == 1 && CU * CV >= 4) return WarpPick<CU, CV, P, 7, PS>::get(); break;   // 2 x 2 tiles of 64 x 64
     }
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -118,6 +119,7 @@ WarpDesc pick_tg(int logs) {
     switch (logs) {
         TGCASE(2) TGCASE(3) TGCASE(4) TGCASE(5)
         case 6: if constexpr (CU * CV >= 4) { TGBODY(6) } break;
+        case 7: if constexpr (CU * CV >= 4) { TGBODY(7) } break;
     }
 #undef TGBODY
 #undef TGCASE
@@ -178,8 +180,8 @@ int derive(grid_plan* p) {
     p->groups_per_cta = 0;
     if (p->variant == 3) {
         const int logs = log2_exact(p->S);
-        if (logs < 2 || logs > 6)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 64], got %d", p->S);
+        if (logs < 2 || logs > 7)
+            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 128], got %d", p->S);
         WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
@@ -209,8 +211,8 @@ int derive(grid_plan* p) {
             return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA may have %d", d.gt, threads);
         p->bin_u = p->bin_v = p->S;
         p->row_u = p->row_v = 2 * p->S;
-        p->nbx = p->S / p->cu;
-        p->nby = p->S / p->cv;
+        p->nbx = (p->S > 64 ? 64 : p->S) / p->cu;          // S = 128: a team covers a 64 x 64 tile of the bin
+        p->nby = (p->S > 64 ? 64 : p->S) / p->cv;
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
@@ -289,7 +291,7 @@ void default_tuning(grid_plan* p) {
     if (p->S < 4) { p->cu = 1; p->cv = 1; }
     // power-of-two supports: bin == support, no padding (grid_warp_kernel.cuh)
     const int logs = log2_exact(p->S);
-    if (logs >= 2 && logs <= 6) {
+    if (logs >= 2 && logs <= 7) {
         grid_plan trial = *p;
         trial.variant = 3;
         trial.threads = 1024;              // clipped to the kernel's register-limited maximum
@@ -304,7 +306,7 @@ void default_tuning(grid_plan* p) {
             else if (logs == 4) { trial.cu = 4; trial.cv = 4; trial.pol_split = 2; }
             else { trial.cu = 4; trial.cv = 2; trial.pol_split = 1; }
         }
-        else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = (logs == 6) ? 4 : 2; }
+        else if (trial.P == 2) { trial.cu = (logs >= 3) ? 4 : 2; trial.cv = (logs >= 6) ? 4 : 2; }
         else if (logs == 2) { trial.cu = 2; trial.cv = 2; }
         else if (logs >= 5) { trial.cu = 8; trial.cv = 4; }
         else { trial.cu = 4; trial.cv = 4; }
@@ -619,6 +621,10 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
             gp.n_groups_b = (gp.n_chunks_b + qt - 1) / qt;
         } else {
             gp.tc = 1; gp.n_tblocks = 1;
+        }
+        if (plan->variant == 3 && plan->S == 128) {              // 2 x 2 tiles per bin: four queue entries per chunk group
+            gp.n_groups_a *= 4;
+            gp.n_groups_b *= 4;
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);

@@ -47,13 +47,15 @@ def test_default_plan_geometry(binding, S, P):
     i = plan.info()
     if i["variant"] == 3:
         # power-of-two support: bin == support, owned positions S/C apart (north_star: "taken modulo the support")
-        assert S in (4, 8, 16, 32) and i["bin_u"] == i["bin_v"] == S
+        assert S in (4, 8, 16, 32, 64, 128) and i["bin_u"] == i["bin_v"] == S
     else:
         # bin >= S + C - 1, aligned to the block; a team covers the bin exactly
         assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
         assert S + i["cu"] - 1 <= i["bin_u"] < S + 2 * i["cu"] - 1
         assert S + i["cv"] - 1 <= i["bin_v"] < S + 2 * i["cv"] - 1
-    assert i["team_threads"] == (i["bin_u"] // i["cu"]) * (i["bin_v"] // i["cv"]) * max(i["pol_split"], 1)
+    tile = min(i["bin_u"], 64) if i["variant"] == 3 else i["bin_u"]      # S = 128: a team covers a 64 x 64 tile
+    tile_v = min(i["bin_v"], 64) if i["variant"] == 3 else i["bin_v"]
+    assert i["team_threads"] == (tile // i["cu"]) * (tile_v // i["cv"]) * max(i["pol_split"], 1)
     assert 1 <= i["teams_per_cta"] <= i["threads_per_cta"] // i["team_threads"]
     assert i["cu"] * i["cv"] * P // max(i["pol_split"], 1) <= 32
     assert i["smem_bytes"] <= 227 * 1024

@@ -220,6 +220,31 @@ def test_support_64(oracle_mod, cu, cv, P, W, mode):
     assert_parity(got, ref, f"S=64 C={cu}x{cv} P={P} W={W} mode={mode} {info}")
 
 
+@pytest.mark.parametrize("cu,cv,P,W", [(8, 4, 1, 2), (4, 4, 1, 2), (4, 2, 4, 2), (4, 4, 2, 2), (2, 2, 1, 2), (8, 4, 1, 40), (4, 2, 4, 40)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_support_128_tiled(oracle_mod, cu, cv, P, W, mode):
+    # S = 128 (the paper's largest bin): the bin is split into 2 x 2 tiles of 64 x 64 positions, one team per
+    # tile, every tile re-reading the chunk; jumps beyond a tile and beyond the support
+    S, O = 128, 2
+    cfg = synth.shrink(synth.get_config("cfg1"), n_ant=6, n_times=19, n_chan=7, grid_size=768)
+    rng = np.random.default_rng(3 * cu + 10 * cv + P)
+    uvw = synth.make_uvw(cfg, rng)
+    n = uvw.shape[0]
+    uvw[:, 2] = rng.uniform(0, W, n)
+    uvw[30:40, :2] = rng.uniform(-300, 300, (10, 2))
+    uvw[50:60, :2] = uvw[49, :2] + rng.uniform(-90, 90, (10, 2))      # jumps around one tile width
+    uvw[40:45, 0] = np.nan
+    vis = (rng.standard_normal((n, P)) + 1j * rng.standard_normal((n, P))).astype(np.complex64)
+    wts = rng.uniform(0.5, 1, n).astype(np.float32)
+    kernel = (rng.standard_normal((W, O, S)) + 1j * rng.standard_normal((W, O, S))).astype(np.complex64)
+    N = cfg.grid_size
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, layout=(cfg.n_baselines, cfg.n_times, cfg.n_chan),
+                        tuning=dict(variant=3, cu=cu, cv=cv, threads_per_cta=1024, batch=16, chunk=64, traversal=mode, time_block=8))
+    assert (info["variant"], info["cu"], info["cv"], info["bin_u"]) == (3, cu, cv, 128)
+    assert_parity(got, ref, f"S=128 C={cu}x{cv} P={P} W={W} mode={mode} {info}")
+
+
 @pytest.mark.parametrize("S,W,P", [(16, 700, 1), (32, 300, 4), (8, 1500, 4), (32, 1229, 1), (4, 4000, 1), (16, 520, 2)])
 def test_tap_table_beyond_shared_memory(oracle_mod, S, W, P):
     # many w-planes (the paper: 1229 per slice): the plan switches to the kernels that read the

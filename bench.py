@@ -285,16 +285,26 @@ def run_ours(args):
     sampler = ClockSampler(local)
     sampler.start()
     launches = 0
+    input_bytes = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4
+    flush_l2 = input_bytes < 2 * 126 * (1 << 20)       # inputs that could sit in the 126 MB L2: flush it between steps
+    if flush_l2:
+        scrub = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        s_events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     ev0.record(stream)
     for k in range(args.steps):
         plan.set_kernel_events(*k_events[k])
+        if flush_l2:
+            scrub.fill_(k & 0xff)                       # outside the step's own event pair
+            s_events[k][0].record(stream)
         step()
+        if flush_l2:
+            s_events[k][1].record(stream)
         launches += plan.last_launches()
     ev1.record(stream)
     barrier()
     clocks = sampler.stop()
     plan.set_kernel_events(None, None)
-    elapsed_ms = ev0.elapsed_time(ev1)
+    elapsed_ms = sum(a.elapsed_time(b) for a, b in s_events) if flush_l2 else ev0.elapsed_time(ev1)
     kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in k_events]))
 
     # ---- end to end: pinned host inputs -> device, execute, grid -> pinned host, every step
@@ -333,8 +343,9 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": cfg.name, "n_vis": cfg.n_vis, "n_valid": n_valid, "grid": N, "support": S,
                        "oversample": O, "n_wplanes": W, "n_pol": P, "updates_per_step": updates_per_step,
-                       "l2": "inputs (%.2f GB per step) exceed the 126 MB L2; no explicit flush" %
-                             ((h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4) / 1e9),
+                       "l2": ("inputs (%.3f GB per step) could stay in the 126 MB L2: a 256 MB buffer is overwritten before "
+                              "every step, outside the step's event pair" if flush_l2 else
+                              "inputs (%.2f GB per step) exceed the 126 MB L2; no explicit flush") % (input_bytes / 1e9),
                        "tuning": info, "compressed": compressed, "op": args.op},
             "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",

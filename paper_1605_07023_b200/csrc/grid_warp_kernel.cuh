@@ -155,7 +155,6 @@ grid_warp_kernel(const GridParams gp) {
     constexpr bool WIDE = S == 32;                     // record format: 32-bit masks need two words
     using mask_t = typename std::conditional<W64, uint64_t, uint32_t>::type;
     static_assert(CU <= TS && CV <= TS, "block larger than the support");
-    static_assert(!DEGRID || T::TEAM <= 32, "degridding: a team must fit one warp (shuffle reduction)");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* staps = reinterpret_cast<float2*>(smem_raw);
@@ -624,7 +623,8 @@ grid_warp_kernel(const GridParams gp) {
                     constexpr int W0 = 2 * PT;
                     uint32_t dup = 0;                          // lane bits over which the result is replicated
 #pragma unroll
-                    for (int o = TEAM / 2, width = W0; o >= 1; o >>= 1) {
+                    constexpr int WT = TEAM < 32 ? TEAM : 32;  // lanes of the team inside this warp
+                    for (int o = WT / 2, width = W0; o >= 1; o >>= 1) {
                         if (width > 1) {
                             const int h = width / 2;
                             const bool hi = (lt & o) != 0;
@@ -643,14 +643,22 @@ grid_warp_kernel(const GridParams gp) {
                             dup |= (uint32_t)o;
                         }
                     }
-                    constexpr int LOGT = TEAM >= 32 ? 5 : TEAM >= 16 ? 4 : TEAM >= 8 ? 3 : TEAM >= 4 ? 2 : TEAM >= 2 ? 1 : 0;
+                    constexpr int LOGT = WT >= 32 ? 5 : WT >= 16 ? 4 : WT >= 8 ? 3 : WT >= 4 ? 2 : WT >= 2 ? 1 : 0;
                     constexpr int WLAST = (W0 >> LOGT) > 1 ? (W0 >> LOGT) : 1;      // floats left per lane
                     const uint32_t code = __float_as_uint(meta.y);
-                    if ((lt & dup) == 0 && code != 0xffffffffu) {
+                    if ((lt & dup & 31) == 0 && code != 0xffffffffu) {
                         float* o = reinterpret_cast<float*>(gp.vis_out + (out_base(my_cg) + (long long)(code & 0x7fffffffu)) * P) + first;
                         const float w = meta.x;
+                        if constexpr (GW > 1 || NT > 1) {
+                            // the team spans several warps (and, at S = 128, four tiles in other groups): every
+                            // warp adds its share atomically; vis_out was zeroed by grid_degrid
 #pragma unroll
-                        for (int i = 0; i < WLAST; ++i) o[i] = (code >> 31) ? 0.f : w * val[i];
+                            for (int i = 0; i < WLAST; ++i)
+                                if (!(code >> 31)) atomicAdd(o + i, w * val[i]);
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < WLAST; ++i) o[i] = (code >> 31) ? 0.f : w * val[i];
+                        }
                     }
                     continue;
                 }

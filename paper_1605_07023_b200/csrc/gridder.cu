@@ -139,11 +139,14 @@ kernel_fn pick_degrid(int logs) {
     switch (logs) {
         case 2: if constexpr (WarpKernelTraits<CU, CV, P, 2>::TEAM <= 32 && CU <= 4 && CV <= 4) return grid_warp_kernel<CU, CV, P, 2, 1, true>; break;
         case 3: if constexpr (WarpKernelTraits<CU, CV, P, 3>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 3, 1, true>; break;
-        case 4: if constexpr (WarpKernelTraits<CU, CV, P, 4>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 4, 1, true>; break;
-        case 5: if constexpr (WarpKernelTraits<CU, CV, P, 5>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 5, 1, true>; break;
+        case 4: if constexpr (WarpKernelTraits<CU, CV, P, 4>::TEAM <= 64) return grid_warp_kernel<CU, CV, P, 4, 1, true>; break;
+        case 5: if constexpr (CU * CV >= 4) return grid_warp_kernel<CU, CV, P, 5, 1, true>; break;    // teams of several warps: atomic combine
     }
     return nullptr;
 }
+
+// multi-warp teams combine through atomics into a zeroed vis_out
+bool degrid_needs_zeroed_output(int cu, int cv, int logs) { return ((1 << logs) / cu) * ((1 << logs) / cv) > 32; }
 
 kernel_fn lookup_degrid(int cu, int cv, int P, int logs) {
 #define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_degrid<a, b, p>(logs);
@@ -754,6 +757,9 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
         for (int t = 0; t < 3; ++t) {
             tmp.cu = tries[t][0]; tmp.cv = tries[t][1];
             if (lookup_degrid(tmp.cu, tmp.cv, tmp.P, logs) && derive(&tmp) == GRID_OK) {
+                if (degrid_needs_zeroed_output(tmp.cu, tmp.cv, logs) &&
+                    cudaMemsetAsync(vis_out, 0, (size_t)plan->n_vis * plan->P * sizeof(float2), stream) != cudaSuccess)
+                    return fail(GRID_ERR_CUDA, "grid_degrid: %s", cudaGetErrorString(cudaGetLastError()));
                 const int rc = execute_impl(&tmp, uvw, nullptr, plan->n_vis, nullptr, weights, conv_kernel,
                                             const_cast<float*>(grid), stream, vis_out);
                 plan->last_launches = tmp.last_launches;

@@ -97,7 +97,7 @@ int grid_execute_compressed(grid_plan* plan, const void* records, const float* v
  *     vis_out[n][p] = weights[n] * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * grid[j0+tj][i0+ti][p]
  * with the same Q, W as grid_execute; skipped samples (R7) get zeros.  <grid_execute(V), G> equals
  * <V, grid_degrid(G)> (pin P7).  grid is read-only; vis_out [n_vis][n_pol] complex64 is overwritten.
- * Two kernels: for power-of-two supports up to 32 the coarsened kernel run backwards -- owned grid values stay in registers while the footprint covers them; otherwise (any
+ * Two kernels: for power-of-two supports up to 128 the coarsened kernel run backwards -- owned grid values stay in registers while the footprint covers them; otherwise (any
  * support) a gather kernel bound by L2 bandwidth.  grid_plan_set_degrid_gather(plan, 1) forces the latter. */
 int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const float* conv_kernel,
                 const float* grid, float* vis_out, grid_stream_t stream);

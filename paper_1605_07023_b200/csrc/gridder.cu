@@ -134,27 +134,33 @@ WarpDesc lookup_warp_tg(int cu, int cv, int P, int logs) {
 }
 
 // Coarsened degridding kernels (grid_warp_kernel<..., DEGRID = true>): teams of at most one warp.
-template <int CU, int CV, int P>
+template <int CU, int CV, int P, bool TGF>
 kernel_fn pick_degrid(int logs) {
     switch (logs) {
-        case 2: if constexpr (WarpKernelTraits<CU, CV, P, 2>::TEAM <= 32 && CU <= 4 && CV <= 4) return grid_warp_kernel<CU, CV, P, 2, 1, true>; break;
-        case 3: if constexpr (WarpKernelTraits<CU, CV, P, 3>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 3, 1, true>; break;
-        case 4: if constexpr (WarpKernelTraits<CU, CV, P, 4>::TEAM <= 64) return grid_warp_kernel<CU, CV, P, 4, 1, true>; break;
-        case 5: if constexpr (CU * CV >= 4) return grid_warp_kernel<CU, CV, P, 5, 1, true>; break;    // teams of several warps: atomic combine
+        case 2: if constexpr (!TGF && WarpKernelTraits<CU, CV, P, 2>::TEAM <= 32 && CU <= 4 && CV <= 4) return grid_warp_kernel<CU, CV, P, 2, 1, true, TGF>; break;
+        case 3: if constexpr (!TGF && WarpKernelTraits<CU, CV, P, 3>::TEAM <= 32) return grid_warp_kernel<CU, CV, P, 3, 1, true, TGF>; break;
+        case 4: if constexpr (WarpKernelTraits<CU, CV, P, 4>::TEAM <= 64) return grid_warp_kernel<CU, CV, P, 4, 1, true, TGF>; break;
+        // teams of several warps (and tiles at S = 128): combined by atomics
+        case 5: if constexpr (CU * CV >= 4) return grid_warp_kernel<CU, CV, P, 5, 1, true, TGF>; break;
+        case 6: if constexpr (CU * CV >= 8) return grid_warp_kernel<CU, CV, P, 6, 1, true, TGF>; break;
+        case 7: if constexpr (CU * CV >= 8) return grid_warp_kernel<CU, CV, P, 7, 1, true, TGF>; break;
     }
     return nullptr;
 }
 
-// multi-warp teams combine through atomics into a zeroed vis_out
-bool degrid_needs_zeroed_output(int cu, int cv, int logs) { return ((1 << logs) / cu) * ((1 << logs) / cv) > 32; }
-
-kernel_fn lookup_degrid(int cu, int cv, int P, int logs) {
-#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_degrid<a, b, p>(logs);
+kernel_fn lookup_degrid(int cu, int cv, int P, int logs, bool tg = false) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return tg ? pick_degrid<a, b, p, true>(logs) : pick_degrid<a, b, p, false>(logs);
     CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
     CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
     CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
 #undef CASE
     return nullptr;
+}
+
+// multi-warp teams (and tiled bins) combine through atomics into a zeroed vis_out
+bool degrid_needs_zeroed_output(int cu, int cv, int logs) {
+    const int ts = (1 << logs) > 64 ? 64 : (1 << logs);
+    return (ts / cu) * (ts / cv) > 32 || logs == 7;
 }
 
 int log2_exact(int v) {
@@ -639,7 +645,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
             gp.gtaps = gt;
             plan->last_launches++;
         }
-        kernel_fn fn = degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs)
+        kernel_fn fn = degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs, plan->taps_global != 0)
                      : (plan->variant == 3 && plan->taps_global) ? lookup_warp_tg(plan->cu, plan->cv, plan->P, logs).fn
                      : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
@@ -748,7 +754,7 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
     if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
         return fail(GRID_ERR_STATE, "grid_degrid: workspace missing or smaller than grid_plan_workspace_bytes()");
     // the coarsened, register-resident kernel where the plan offers one; the gather kernel otherwise
-    if (plan->variant == 3 && plan->degrid_gather == 0 && !plan->taps_global) {
+    if (plan->variant == 3 && plan->degrid_gather == 0) {
         grid_plan tmp = *plan;                       // same plan with polarisation split 1 (shuffle reduction per team)
         tmp.pol_split = 1;
         tmp.threads = 1024;
@@ -756,7 +762,8 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
         const int tries[3][2] = {{plan->cu, plan->cv}, {4, 2}, {2, 2}};
         for (int t = 0; t < 3; ++t) {
             tmp.cu = tries[t][0]; tmp.cv = tries[t][1];
-            if (lookup_degrid(tmp.cu, tmp.cv, tmp.P, logs) && derive(&tmp) == GRID_OK) {
+            if (derive(&tmp) == GRID_OK && tmp.taps_global == plan->taps_global &&      // same workspace layout
+                lookup_degrid(tmp.cu, tmp.cv, tmp.P, logs, tmp.taps_global != 0)) {
                 if (degrid_needs_zeroed_output(tmp.cu, tmp.cv, logs) &&
                     cudaMemsetAsync(vis_out, 0, (size_t)plan->n_vis * plan->P * sizeof(float2), stream) != cudaSuccess)
                     return fail(GRID_ERR_CUDA, "grid_degrid: %s", cudaGetErrorString(cudaGetLastError()));

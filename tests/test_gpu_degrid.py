@@ -55,6 +55,23 @@ def test_degrid_matches_oracle(oracle_mod, S, P):
     assert np.linalg.norm(got - ref) <= 1e-5 * np.linalg.norm(ref)
 
 
+@pytest.mark.parametrize("S,P,W", [(64, 1, 2), (64, 4, 2), (128, 1, 2), (128, 4, 2), (32, 4, 300), (16, 1, 700), (64, 4, 40), (128, 1, 40)])
+def test_degrid_large_supports_and_tables(oracle_mod, S, P, W):
+    # degridding with multi-warp teams, tiled bins (S = 128) and tap tables in global memory (many planes)
+    N, O, n = 640, 2, 6_007
+    uvw, _, wts, kernel = synth.random_problem(300 + S + P + W, n, N, S, O, W, P, spread=0.4, walk=2.0)
+    uvw[20:30, 0] = np.nan
+    rng = np.random.default_rng(S + W)
+    grid = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+    ref = oracle_mod.degrid(N, S, O, W, P, uvw, wts, kernel, grid)
+    got = gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid).astype(np.complex128)
+    via_gather = gpu_degrid(N, S, O, W, P, uvw, wts, kernel, grid, gather=True).astype(np.complex128)
+    assert not got[20:30].any()
+    assert np.linalg.norm(got - ref) <= 1e-5 * np.linalg.norm(ref)
+    assert np.linalg.norm(via_gather - ref) <= 1e-5 * np.linalg.norm(ref)
+    assert np.abs(got - ref).max() <= 2e-5 * np.sqrt(np.mean(np.abs(ref) ** 2)) * max(1.0, S / 8)
+
+
 def test_adjoint_identity_on_gpu(oracle_mod):
     # <grid(V), G> == <V, degrid(G)> with both operators on the GPU (pin P7's identity for the CUDA pair)
     N, S, O, W, P, n = 256, 8, 8, 2, 4, 20_000

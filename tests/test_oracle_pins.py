@@ -378,3 +378,26 @@ def test_compress_oracle_runs_and_invariance(oracle_mod):
     g_c = oracle_mod.grid(N, S, O, W, 2, uvw[heads], merged.astype(np.complex64), np.ones(len(heads), np.float32),
                           np.ones((W, O, S), np.complex64) * (1 + 0.5j))
     np.testing.assert_allclose(g_c, g, rtol=1e-12, atol=1e-12)
+
+
+def test_dense_oracle_unit_sample_and_separable_limit(oracle_mod):
+    # oracle.grid_dense (NEXT-4): (a) one unit visibility reproduces kernel2d[wp][sv][su] with rows = v taps and
+    # columns = u taps, at the cell the quantiser gives (hand-placed, asymmetric table so a transpose shows);
+    # (b) a dense table that IS an outer product gives exactly the separable oracle's grid
+    rng = np.random.default_rng(33)
+    k2 = (rng.standard_normal((W, O, O, S, S)) + 1j * rng.standard_normal((W, O, O, S, S))).astype(np.complex64)
+    uvw = np.array([[3.0, -4.25, 1.5]], dtype=np.float32)      # Q by hand (N=32, S=5, O=4): su = (12+58) % 4 = 2, sv = (-17+58) % 4 = 1
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    assert (q["su"][0], q["sv"][0], q["wp"][0]) == (2, 1, 1)
+    g = oracle_mod.grid_dense(N, S, O, W, 1, uvw, np.ones((1, 1), np.complex64), np.ones(1, np.float32), k2)
+    expect = np.zeros((N, N), np.complex128)
+    expect[q["j0"][0]:q["j0"][0] + S, q["i0"][0]:q["i0"][0] + S] = k2[1, 1, 2].astype(np.complex128)
+    np.testing.assert_array_equal(g[:, :, 0], expect)
+    uvw, vis, wts, kernel = synth.random_problem(34, 700, N, S, O, W, 2, spread=0.5)
+    kk = kernel.astype(np.complex128)
+    outer = (kk[:, :, None, :, None] * kk[:, None, :, None, :])        # [wp][sv][su][tj][ti] = k[wp][sv][tj] * k[wp][su][ti]
+    g_sep = oracle_mod.grid(N, S, O, W, 2, uvw, vis, wts, kernel)
+    # the outer product is not exactly representable in complex64: compare through the rounded table's own error
+    g_dense = oracle_mod.grid_dense(N, S, O, W, 2, uvw, vis, wts, outer.astype(np.complex64))
+    assert np.abs(g_dense - g_sep).max() <= 4e-7 * np.abs(g_sep).max()
+    assert np.linalg.norm(g_dense - g_sep) <= 2e-7 * np.linalg.norm(g_sep)

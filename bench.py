@@ -38,8 +38,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--op", default="grid", choices=["grid", "degrid"],
-                    help="degrid: time grid_degrid (the adjoint, SURVEY NEXT-2) instead of grid_execute")
+    ap.add_argument("--op", default="grid", choices=["grid", "degrid", "dense"],
+                    help="degrid: time grid_degrid (the adjoint, SURVEY NEXT-2); dense: time grid_execute_dense with the "
+                         "outer product of the separable taps as a non-separable table (NEXT-4); default grid_execute")
     ap.add_argument("--compressed", action="store_true",
                     help="compress once outside the timed region (PAPER.md:69, 113) and time grid_execute_compressed; "
                          "the rate then counts compressed samples, as the paper's does")
@@ -256,8 +257,15 @@ def run_ours(args):
         grid.copy_(torch.randn((N, N, P), dtype=torch.complex64, device=dev))
         kernel_name = "grid_degrid: grid_warp_kernel<..,DEGRID> where a team fits a warp, else degrid_gather_kernel"
 
+    d_k2 = None
+    if args.op == "dense":                                     # [W][O][O][S][S] = k[wp][sv][tj] * k[wp][su][ti]
+        d_k2 = (d_kern[:, :, None, :, None] * d_kern[:, None, :, None, :]).contiguous()
+        kernel_name = "grid_execute_dense: grid_warp_kernel<..,DENSE> (S <= 32), else grid_scatter_dense_kernel"
+
     def step():
-        if d_out is not None:
+        if d_k2 is not None:
+            plan.execute_dense(d_uvw, d_vis, d_wts, d_k2, grid)
+        elif d_out is not None:
             plan.degrid(d_uvw, d_wts, d_kern, grid, d_out)
         elif compressed:
             plan.execute_compressed(c_recs, c_vis, d_kern, grid)
@@ -309,7 +317,7 @@ def run_ours(args):
 
     # ---- end to end: pinned host inputs -> device, execute, grid -> pinned host, every step
     e2e = None
-    if not args.no_e2e and not compressed and d_out is None:
+    if not args.no_e2e and not compressed and d_out is None and d_k2 is None:
         h_grid = torch.empty((N, N, P), dtype=torch.complex64).pin_memory()
         e_steps = max(3, min(args.steps, 10))
         h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4

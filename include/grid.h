@@ -92,6 +92,16 @@ int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const flo
 int grid_execute_compressed(grid_plan* plan, const void* records, const float* vis, long long n,
                             const float* conv_kernel, float* grid, grid_stream_t stream);
 
+/* Gridding with a dense (non-separable) GCF table (A-projection-like kernels; the paper
+ * expects smaller gains there and does not measure it):
+ *     grid[j0+tj][i0+ti][p] += weights[n] * vis[n][p] * conv_kernel_2d[wp][sv][su][tj][ti]
+ *   conv_kernel_2d  [n_wplanes][oversample][oversample][support][support] complex64, DEVICE
+ * Everything else as grid_execute (same Q, W, skipping rule, accumulation).  Power-of-two supports up to
+ * 32 run on the coarsened kernel with the table read through L1/L2; other supports on a
+ * one-atomic-per-update kernel. */
+int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                       const float* conv_kernel_2d, float* grid, grid_stream_t stream);
+
 /* Degridding, the adjoint of grid_execute (the paper calls its own degridder preliminary
  * and does not measure it).  For every sample whose footprint lies inside the grid
  *     vis_out[n][p] = weights[n] * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * grid[j0+tj][i0+ti][p]

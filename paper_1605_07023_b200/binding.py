@@ -15,7 +15,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
-    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
     "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
@@ -36,6 +36,7 @@ _lib.grid_plan_set_workspace.argtypes = [_vp, _vp, _sz]
 _lib.grid_execute.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
 _lib.grid_compress.argtypes = [_vp] * 8
+_lib.grid_execute_dense.argtypes = [_vp] * 7
 _lib.grid_degrid.argtypes = [_vp] * 7
 _lib.grid_plan_set_degrid_gather.argtypes = [_vp, _int]
 _lib.grid_execute_compressed.argtypes = [_vp, _vp, _vp, _ll, _vp, _vp, _vp]
@@ -172,6 +173,17 @@ class GridPlan:
                                _ptr(conv_kernel, torch.complex64, "conv_kernel"),
                                _ptr(grid, torch.complex64, "grid"), _stream(stream))
         _check(rc, "grid_execute")
+
+    def execute_dense(self, uvw, vis, weights, conv_kernel_2d, grid, stream=None):
+        """grid_execute_dense: conv_kernel_2d complex64 [W][O][O][S][S] (plane, sv, su, row, column)."""
+        import torch
+        if conv_kernel_2d.numel() != self.n_wplanes * self.oversample ** 2 * self.support ** 2:
+            raise ValueError("conv_kernel_2d must be [n_wplanes][oversample][oversample][support][support]")
+        rc = _lib.grid_execute_dense(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
+                                     _ptr(weights, torch.float32, "weights"),
+                                     _ptr(conv_kernel_2d, torch.complex64, "conv_kernel_2d"),
+                                     _ptr(grid, torch.complex64, "grid"), _stream(stream))
+        _check(rc, "grid_execute_dense")
 
     def compress(self, uvw, vis, weights, stream=None):
         """grid_compress: returns (records uint8 [n_c][8], vis complex64 [n_c][P], n_c) -- CUDA tensors trimmed

@@ -142,7 +142,10 @@ struct WarpKernelTraits {
 // TG: the tap table does not fit shared memory (many w-planes: the paper uses 1229 per slice,
 // PAPER.md:113) -- taps are read through L1/L2 from a row-doubled copy in global memory (gp.gtaps),
 // as the paper's kernel does (Table 1 "unified cache").
-template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false, bool TG = false>
+// DENSE: gp.kern is a non-separable table [W][O][O][S][S]
+// (plane, v sub-offset, u sub-offset, row, column); a thread fetches the Cu*Cv values of its points from
+// global memory (L1/L2) instead of Cu+Cv taps, and no GCF product is formed.  S <= 32.
+template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false, bool TG = false, bool DENSE = false>
 __global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS, PS>::MAX_THREADS), 1)
 grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
@@ -152,13 +155,14 @@ grid_warp_kernel(const GridParams gp) {
     static_assert(NT == 1 || TPG == 1, "tiled bins: one team per group");
     constexpr int ROW = 2 * S;                         // doubled tap row k[t mod S], t < 2S: offsets reach 2S-1
     constexpr bool W64 = T::W64;                       // S = 64: {pos, tap rows, -, -} + a mask record {mx, my} of 64 bits each
-    constexpr bool WIDE = S == 32;                     // record format: 32-bit masks need two words
+    constexpr bool WIDE = S == 32 || (DENSE && S < 32); // record format: masks in two words
+    static_assert(!DENSE || (S <= 32 && !DEGRID && !TG), "dense tables: S <= 32, gridding only");
     using mask_t = typename std::conditional<W64, uint64_t, uint32_t>::type;
     static_assert(CU <= TS && CV <= TS, "block larger than the support");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* staps = reinterpret_cast<float2*>(smem_raw);
-    const size_t taps_bytes = TG ? 0 : ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
+    const size_t taps_bytes = (TG || DENSE) ? 0 : ((size_t)gp.n_rows * ROW * sizeof(float2) + 15) & ~(size_t)15;
     const int B = gp.batch, bshift = gp.batch_shift;
     const int slots = TPG * B;
 
@@ -175,7 +179,7 @@ grid_warp_kernel(const GridParams gp) {
     uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
     uint32_t* ctrl = last_pos + 2 * TPG;
 
-    if constexpr (!TG) {
+    if constexpr (!TG && !DENSE) {
         for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {      // a4
             const int r = k / ROW, t = (k - r * ROW) & (S - 1);
             staps[k] = __ldg(gp.kern + (size_t)r * S + t);
@@ -434,7 +438,13 @@ grid_warp_kernel(const GridParams gp) {
                 const uint32_t xo = (rec.rows & 0xffffu) * ROW + S - (i0 & (S - 1));
                 const uint32_t yo = (rec.rows >> 16) * ROW + S - (j0 & (S - 1));
                 c.x = rec.pos & 0xffff7fffu;
-                if constexpr (W64) {
+                if constexpr (DENSE) {
+                    // table row ((wp*O + sv)*O + su), in elements of S*S
+                    const uint32_t ru = rec.rows & 0xffffu, rv = rec.rows >> 16;
+                    const uint32_t su = ru - (ru / (uint32_t)gp.oversample) * (uint32_t)gp.oversample;
+                    c.y = (rv * (uint32_t)gp.oversample + su) * (uint32_t)(S * S);
+                    c.z = mx; c.w = my;
+                } else if constexpr (W64) {
                     c.y = rec.rows;
                     cmask[kk] = make_uint4((uint32_t)mx, (uint32_t)((uint64_t)mx >> 32), (uint32_t)my, (uint32_t)((uint64_t)my >> 32));
                 }
@@ -570,6 +580,31 @@ grid_warp_kernel(const GridParams gp) {
                         }
                     }
                     }
+                }
+                if constexpr (DENSE) {
+                    const int mi = (px0 - (int)(c.x & 0x7fffu)) & (S - 1), mj = (py0 - (int)(c.x >> 16)) & (S - 1);
+                    const float2* kb = gp.kern + c.y;
+                    float2 g2[CV][CU], v[PT];
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                        for (int a = 0; a < CU; ++a)
+                            g2[bb][a] = __ldg(kb + ((mj + bb * DV) & (S - 1)) * S + ((mi + a * DU) & (S - 1)));
+#pragma unroll
+                    for (int q = 0; q < PT; ++q) v[q] = vp[q];
+                    vp += P;
+#pragma unroll
+                    for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                        for (int a = 0; a < CU; ++a)
+#pragma unroll
+                            for (int q = 0; q < PT; ++q) {                                   // a7
+                                acc[bb][a][q].x = fmaf(g2[bb][a].x, v[q].x, acc[bb][a][q].x);
+                                acc[bb][a][q].x = fmaf(-g2[bb][a].y, v[q].y, acc[bb][a][q].x);
+                                acc[bb][a][q].y = fmaf(g2[bb][a].x, v[q].y, acc[bb][a][q].y);
+                                acc[bb][a][q].y = fmaf(g2[bb][a].y, v[q].x, acc[bb][a][q].y);
+                            }
+                    continue;
                 }
                 const float2* tu;
                 const float2* tv;

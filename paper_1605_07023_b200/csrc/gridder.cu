@@ -44,6 +44,7 @@ struct grid_plan {
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
     int groups_per_cta, queue_teams;
+    int dense;                            // internal (grid_execute_dense): non-separable table, read from global memory
     int taps_global;                      // variant 3: tap table read from global memory (too large for shared)
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
@@ -133,6 +134,51 @@ WarpDesc lookup_warp_tg(int cu, int cv, int P, int logs) {
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
+// Dense (non-separable) GCF kernels: default blocks, S <= 32.
+template <int CU, int CV, int P>
+WarpDesc pick_dense(int logs) {
+#define DCASE(l) case l: if constexpr (CU <= (1 << l) && CV <= (1 << l)) { using T = WarpKernelTraits<CU, CV, P, l, 1>; \
+        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; } break;
+    switch (logs) { DCASE(2) DCASE(3) DCASE(4) DCASE(5) }
+#undef DCASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+WarpDesc lookup_warp_dense(int cu, int cv, int P, int logs) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_dense<a, b, p>(logs);
+    CASE(2, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1) CASE(2, 2, 2) CASE(4, 2, 2) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+// Dense GCF, any support: one thread per (sample, footprint row), one atomic per update (fallback).
+template <int P>
+__global__ void __launch_bounds__(256)
+grid_scatter_dense_kernel(const CycRec* __restrict__ recs, const float2* __restrict__ vis, const float* __restrict__ weights,
+                          const float2* __restrict__ kernel2d, float* __restrict__ grid, long long n_vis, int N, int S, int O) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = g / S;
+    const int tj = (int)(g - n * S);
+    if (n >= n_vis) return;
+    const CycRec rec = recs[n];
+    if (rec.pos & 0x8000u) return;
+    const int i0 = (int)(rec.pos & 0x7fffu), j0 = (int)(rec.pos >> 16);
+    const uint32_t ru = rec.rows & 0xffffu, rv = rec.rows >> 16;
+    const uint32_t su = ru - (ru / (uint32_t)O) * (uint32_t)O;
+    const float2* k = kernel2d + ((size_t)rv * O + su) * S * S + (size_t)tj * S;
+    const float w = weights[n];
+    float* row = grid + ((size_t)(j0 + tj) * N + i0) * (2 * P);
+    for (int ti = 0; ti < S; ++ti) {
+        const float2 gk = __ldg(k + ti);
+#pragma unroll
+        for (int q = 0; q < P; ++q) {
+            float2 v = vis[n * P + q];
+            v.x *= w; v.y *= w;
+            red_add_v2(row + (size_t)(ti * P + q) * 2, gk.x * v.x - gk.y * v.y, gk.x * v.y + gk.y * v.x);
+        }
+    }
+}
+
 // Coarsened degridding kernels (grid_warp_kernel<..., DEGRID = true>): teams of at most one warp.
 template <int CU, int CV, int P, bool TGF>
 kernel_fn pick_degrid(int logs) {
@@ -195,11 +241,18 @@ int derive(grid_plan* p) {
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
                         p->cu, p->cv, p->pol_split, p->P, p->S);
+        if (p->dense) {                                  // grid_execute_dense: no tap table on chip
+            d = lookup_warp_dense(p->cu, p->cv, p->P, logs);
+            if (!d.fn || p->pol_split != 1)
+                return fail(GRID_ERR_UNSUPPORTED, "dense GCF: block %dx%d is not instantiated for %d pols, support %d",
+                            p->cu, p->cv, p->P, p->S);
+        }
         // Tap table: in shared memory when it leaves at least half of it to the warp groups (and, for S = 32,
         // its offsets fit the record's 16 bits); otherwise read through L1/L2 from global memory (TG kernels).
         size_t taps = ((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15;
         p->taps_global = 0;
-        if (taps > (size_t)p->max_smem / 2 || taps + d.group_bytes(p->batch) > (size_t)p->max_smem ||
+        if (p->dense) taps = 0;
+        else if (taps > (size_t)p->max_smem / 2 || taps + d.group_bytes(p->batch) > (size_t)p->max_smem ||
             (logs == 5 && (long long)p->W * p->O * 2 * p->S > 65535)) {
             const WarpDesc g = p->pol_split == 1 ? lookup_warp_tg(p->cu, p->cv, p->P, logs) : WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
             if (!g.fn)
@@ -565,6 +618,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.counters = counters;
     gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
+    gp.oversample = plan->O;
     gp.bin_u = plan->bin_u; gp.bin_v = plan->bin_v; gp.row_u = plan->row_u; gp.row_v = plan->row_v;
     gp.nbx = plan->nbx; gp.nby = plan->nby;
     gp.team_threads = plan->team_threads; gp.teams_per_cta = plan->teams_per_cta;
@@ -637,7 +691,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
         const int logs = log2_exact(plan->S);
-        if (plan->variant == 3 && plan->taps_global) {           // a4: row-doubled table in global memory
+        if (plan->variant == 3 && plan->taps_global && !plan->dense) {   // a4: row-doubled table in global memory
             float2* gt = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes +
                                                    records_bytes(plan) + ((order_capacity(plan) * sizeof(uint32_t) + 15) & ~(size_t)15));
             const long long n_elems = (long long)plan->W * plan->O * 2 * plan->S;
@@ -645,7 +699,8 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
             gp.gtaps = gt;
             plan->last_launches++;
         }
-        kernel_fn fn = degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs, plan->taps_global != 0)
+        kernel_fn fn = plan->dense ? lookup_warp_dense(plan->cu, plan->cv, plan->P, logs).fn
+                     : degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs, plan->taps_global != 0)
                      : (plan->variant == 3 && plan->taps_global) ? lookup_warp_tg(plan->cu, plan->cv, plan->P, logs).fn
                      : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
@@ -797,6 +852,58 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
     plan->last_launches = 2;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_degrid: launch failed: %s", cudaGetErrorString(e));
+    return GRID_OK;
+}
+
+int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                       const float* conv_kernel_2d, float* grid, grid_stream_t stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute_dense: call grid_plan_set_samples first");
+    if (plan->n_vis == 0) return GRID_OK;
+    if (!uvw || !vis || !weights || !conv_kernel_2d || !grid)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: null array argument");
+    if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel_2d | (uintptr_t)grid) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: array arguments must be 16-byte aligned");
+    if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
+        return fail(GRID_ERR_STATE, "grid_execute_dense: workspace missing or smaller than grid_plan_workspace_bytes()");
+    if ((long long)plan->W * plan->O * plan->O * plan->S * plan->S > 0x7fffffffLL)
+        return fail(GRID_ERR_UNSUPPORTED, "grid_execute_dense: table beyond 2^31 elements");
+    const int logs = log2_exact(plan->S);
+    if (logs >= 2 && logs <= 5) {                    // coarsened kernel with the default block of this (S, P)
+        grid_plan tmp = *plan;
+        tmp.variant = 3; tmp.dense = 1; tmp.pol_split = 1; tmp.threads = 1024; tmp.batch = 32; tmp.chunk = 256;
+        if (tmp.P == 1) { tmp.cu = logs == 2 ? 2 : (logs == 5 ? 8 : 4); tmp.cv = logs == 2 ? 2 : 4; }
+        else if (tmp.P == 2) { tmp.cu = logs == 2 ? 2 : 4; tmp.cv = 2; }
+        else { tmp.cu = logs <= 3 ? 2 : 4; tmp.cv = 2; }
+        if (derive(&tmp) == GRID_OK) {               // uses a subset of the plan's workspace (no tap table copy)
+            const int rc = execute_impl(&tmp, uvw, nullptr, plan->n_vis, vis, weights, conv_kernel_2d, grid, stream);
+            plan->last_launches = tmp.last_launches;
+            return rc;
+        }
+        g_err[0] = 0;
+    }
+    // any other support: one atomic per update
+    const long long n = plan->n_vis;
+    if (n * plan->S / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_execute_dense: too many samples");
+    unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
+    CycRec* recs = reinterpret_cast<CycRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
+    if (cudaMemsetAsync(counters, 0, 256, stream) != cudaSuccess)
+        return fail(GRID_ERR_CUDA, "grid_execute_dense: %s", cudaGetErrorString(cudaGetLastError()));
+    QuantParams qp = quant_params(plan);
+    qp.format = 1;
+    quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
+        uvw, reinterpret_cast<SampleRec*>(recs), n, qp, reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
+    const unsigned blocks = (unsigned)((n * plan->S + 255) / 256);
+    const float2* v2 = reinterpret_cast<const float2*>(vis);
+    const float2* k2 = reinterpret_cast<const float2*>(conv_kernel_2d);
+    if (plan->P == 1) grid_scatter_dense_kernel<1><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
+    else if (plan->P == 2) grid_scatter_dense_kernel<2><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
+    else grid_scatter_dense_kernel<4><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
+    plan->last_launches = 2;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute_dense: launch failed: %s", cudaGetErrorString(e));
     return GRID_OK;
 }
 

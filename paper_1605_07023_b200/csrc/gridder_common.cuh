@@ -44,6 +44,7 @@ struct GridParams {
     long long n_vis;
     long long n_groups_a, n_groups_b, n_chunks_b;   // mode 0 / mode 1 work decomposition
     int N, S, n_rows;         // n_rows = W*O
+    int oversample;           // O (dense tables: row = (wp*O + sv)*O + su)
     int bin_u, bin_v, row_u, row_v, nbx, nby;
     int team_threads, teams_per_cta, batch, chunk, batch_shift;
     int groups_per_cta;       // variant 3: warp groups per CTA (each its own queue consumer)

@@ -127,7 +127,7 @@ struct WarpKernelTraits {
     static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
     // shared memory of one group for a batch of B samples per team
     static constexpr bool W64 = TS == 64;                 // 64-bit moved masks live in a second 16-byte record
-    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * B * (16 + (W64 ? 16 : 0) + 8 * P); }
+    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * (B + 1) * (16 + (W64 ? 16 : 0) + 8 * P); }   // team stride B + 1 slots: see BP
     __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
     __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
     __host__ __device__ static constexpr size_t group_bytes(int B) {
@@ -169,9 +169,15 @@ grid_warp_kernel(const GridParams gp) {
     const int tid = threadIdx.x;
     const int group = tid / GT, lg = tid - group * GT;
     unsigned char* gbase = smem_raw + taps_bytes + (size_t)group * T::group_bytes(B);
+    // Cooked arrays: the teams of a group are B + 1 slots apart, so that the same sample slot of two teams
+    // falls into different banks (a stride of B slots is a multiple of 128 bytes: every record and
+    // visibility load of the hot loop was a 2-way bank conflict, 34 % of all shared wavefronts on cfg1).
+    // The extra slot is also the slack the hot loop's read-ahead of the next record needs.
+    const int BP = B + 1;
+    const int cslots = TPG * BP;
     uint4* crec = reinterpret_cast<uint4*>(gbase);                                       // cooked records
-    float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)slots * 16);                // cooked vis
-    uint4* cmask = reinterpret_cast<uint4*>(gbase + (size_t)slots * (16 + 8 * P));       // W64 only
+    float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)cslots * 16);               // cooked vis
+    uint4* cmask = reinterpret_cast<uint4*>(gbase + (size_t)cslots * (16 + 8 * P));      // W64 only
     unsigned char* rbase = gbase + T::cooked_bytes(B);
     const size_t rstage = T::raw_bytes(B);
     // raw stage layout: vis [slots][P] float2, rec [slots] 8 B, weights [slots] float
@@ -204,9 +210,9 @@ grid_warp_kernel(const GridParams gp) {
 #pragma unroll
     for (int b = 0; b < CV; ++b) MY |= mask_t(1) << (s0 + b * DV);
     const uint32_t MXY = (uint32_t)MX | ((uint32_t)MY << 16);      // S <= 16: both masks in one word
-    const uint4* my_mask = cmask + (size_t)tg * B;
-    const uint4* my_rec = crec + (size_t)tg * B;
-    const float2* my_vis = cvis + (size_t)tg * B * P + (DEGRID ? 0 : half * PT);   // DEGRID: {weight, sample code}
+    const uint4* my_mask = cmask + (size_t)tg * BP;
+    const uint4* my_rec = crec + (size_t)tg * BP;
+    const float2* my_vis = cvis + (size_t)tg * BP * P + (DEGRID ? 0 : half * PT);   // DEGRID: {weight, sample code}
     const unsigned char* my_tu;
     const unsigned char* my_tv;
     if constexpr (TG) {
@@ -237,11 +243,13 @@ grid_warp_kernel(const GridParams gp) {
     float* gridp = gp.grid;
     asm volatile("" : "+l"(gridp));
 
-    // (clearing by a reload of zeros from shared memory was tried: ptxas still copies the loaded
-    //  registers into the accumulators one by one, so plain assignments are kept)
+    // Clearing a flushed point: 2*PT moves from a zero the compiler cannot see (gp.fzero, constant bank).  With a
+    // literal 0.f ptxas rebuilds four uniform zero registers inside every flush body.  Measured and not kept
+    // (profiles/r2_flush_experiments.md): clearing by LDS.128 of zeros (fewer issue slots, but the shared-memory
+    // pipe is the second limit of this kernel), clearing by FFMAs of hidden zeros (ptxas folds or hoists them).
     auto clear_point = [&](float2 (&v)[PT]) {
 #pragma unroll
-        for (int q = 0; q < PT; ++q) v[q] = make_float2(0.f, 0.f);
+        for (int q = 0; q < PT; ++q) v[q] = make_float2(gp.fzero, gp.fzero);
     };
 
     // DEGRID: fetch the value of a grid point my team now covers
@@ -416,7 +424,8 @@ grid_warp_kernel(const GridParams gp) {
             uint4 c = make_uint4(0u, 0u, 0u, 0u);
             float w = 0.f;
             bool valid = false;
-            if constexpr (W64) cmask[kk] = make_uint4(0u, 0u, 0u, 0u);
+            const int ck = t * BP + k;                 // slot in the cooked arrays
+            if constexpr (W64) cmask[ck] = make_uint4(0u, 0u, 0u, 0u);
             if (k < cnt) {
                 const CycRec rec = rrec[kk];
                 mask_t mx = 0, my = 0;
@@ -446,7 +455,7 @@ grid_warp_kernel(const GridParams gp) {
                     c.z = mx; c.w = my;
                 } else if constexpr (W64) {
                     c.y = rec.rows;
-                    cmask[kk] = make_uint4((uint32_t)mx, (uint32_t)((uint64_t)mx >> 32), (uint32_t)my, (uint32_t)((uint64_t)my >> 32));
+                    cmask[ck] = make_uint4((uint32_t)mx, (uint32_t)((uint64_t)mx >> 32), (uint32_t)my, (uint32_t)((uint64_t)my >> 32));
                 }
                 else if constexpr (WIDE && TG) { c.y = rec.rows; c.z = mx; c.w = my; }     // offsets exceed 16 bits
                 else if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
@@ -454,18 +463,18 @@ grid_warp_kernel(const GridParams gp) {
                 valid = (rec.pos & 0x8000u) == 0;
                 if (valid) w = gp.weights ? rw[kk] : 1.f;
             }
-            crec[kk] = c;
+            crec[ck] = c;
             if constexpr (DEGRID) {
                 // where the result goes: offset from the chunk base, bit 31 = skipped sample, all ones = no sample
                 uint32_t code = 0xffffffffu;
                 if (k < cnt) code = (uint32_t)(sample_of(cg, b, k) - out_base(cg)) | (valid ? 0u : 0x80000000u);
-                cvis[(size_t)kk * P] = make_float2(w, __uint_as_float(code));
+                cvis[(size_t)ck * P] = make_float2(w, __uint_as_float(code));
             } else {
 #pragma unroll
                 for (int q = 0; q < P; ++q) {
                     float2 v = make_float2(0.f, 0.f);
                     if (valid) { v = rvis[(size_t)kk * P + q]; v.x *= w; v.y *= w; }
-                    cvis[(size_t)kk * P + q] = v;
+                    cvis[(size_t)ck * P + q] = v;
                 }
             }
         }
@@ -516,10 +525,10 @@ grid_warp_kernel(const GridParams gp) {
 
             const uint4* rp = my_rec;
             const float2* vp = my_vis;
-            uint4 c_next = *rp;
+            uint4 c = *rp;
             for (int s = 0; s < cnt; ++s) {
-                const uint4 c = c_next;
-                c_next = *++rp;                        // next record (one slot of slack follows the batch)
+                // (the next record is loaded into the same registers once this one's fields have been consumed,
+                //  below: no register rotation at the loop head; one slot of slack follows the batch)
                 bool moved;
                 mask_t mx_all = 0, my_all = 0;             // this sample's moved masks
                 if constexpr (W64) {
@@ -584,6 +593,7 @@ grid_warp_kernel(const GridParams gp) {
                 if constexpr (DENSE) {
                     const int mi = (px0 - (int)(c.x & 0x7fffu)) & (S - 1), mj = (py0 - (int)(c.x >> 16)) & (S - 1);
                     const float2* kb = gp.kern + c.y;
+                    c = *++rp;                         // next sample's record
                     float2 g2[CV][CU], v[PT];
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb)
@@ -618,6 +628,7 @@ grid_warp_kernel(const GridParams gp) {
                     tu = reinterpret_cast<const float2*>(my_tu + c.y);
                     tv = reinterpret_cast<const float2*>(my_tv + c.z);
                 }
+                c = *++rp;                             // next sample's record
                 float2 gu[CU], gv[CV], v[PT];
 #pragma unroll
                 for (int a = 0; a < CU; ++a) gu[a] = tu[a * DU];

@@ -55,6 +55,7 @@ struct GridParams {
     int tile_shift;           // log2 of the tile side used for that order
     int n_cblocks, chunk_cols;   // variant 3, time-innermost: a chunk spans chunk_cols channels
     int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
+    float fzero;              // 0.0f the compiler cannot see: accumulators are cleared by moves from the constant bank
 };
 
 }  // namespace gridb200

@@ -16,7 +16,9 @@ from gpu_util import REL_L2_TOL, MAX_ABS_TOL
 
 pytestmark = pytest.mark.gpu
 
-FULL = ["cfg1", "cfg2", "cfg3", "cfg4_S4_P1", "cfg4_S32_P4", "cfg4_S16_P1"]
+# every BASELINE.json config and all eight points of the config-4 sweep, each with the plan's default tuning
+FULL = ["cfg1", "cfg2", "cfg3", "cfg4_S4_P1", "cfg4_S4_P4", "cfg4_S8_P1", "cfg4_S8_P4", "cfg4_S16_P1", "cfg4_S16_P4",
+        "cfg4_S32_P1", "cfg4_S32_P4"]
 
 
 def _bands(N, S):

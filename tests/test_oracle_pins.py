@@ -180,7 +180,10 @@ def test_p6_whole_cell_translation(oracle_mod):
     sh[:, 1] -= 2.0
     g1 = oracle_mod.grid(48, S, O, W, 2, sh, vis, wts, kernel)
     assert np.array_equal(g1[:-2, 1:], g0[2:, :-1])       # bit-for-bit
-    assert np.count_nonzero(g1[:, 0]) == 0 or True
+    # what slid in from outside the grid is empty: column 0 (u + 1) and the last two rows (v - 2)
+    assert np.count_nonzero(g1[:, 0]) == 0 and np.count_nonzero(g1[-2:, :]) == 0
+    # and nothing was lost at the far edges of the original
+    assert np.count_nonzero(g0[:, -1]) == 0 and np.count_nonzero(g0[:2, :]) == 0
 
 
 @pytest.mark.parametrize("P", [1, 4])
@@ -338,6 +341,38 @@ def test_quantise_matches_independent_python(oracle_mod):
             else:
                 assert q["valid"][k] == 0
             assert j_ok or q["valid"][k] == 0
+
+
+def test_r4_odd_oversample_times_support_by_hand(oracle_mod):
+    """R4 for odd O*S with O > 1, worked on paper for (N, S, O) = (64, 5, 3) (R4 and R8).
+
+    Centre cell 32; the sample is snapped to the nearest 1/3 cell, ties up, and the S = 5 cells of its
+    footprint are those at distance d in (-2.5, 2.5] of the snapped position (R8).  Nothing below uses the
+    oracle's shift constant O - ceil(O*S/2):
+      x = +0.4   -> x*3 = 1.2   -> nearest third 1/3      -> position 32 1/3: cells 30..34 (29 is 3 1/3 away, 35 is 2 2/3) -> i0 = 30
+      x =  0.0   ->                nearest third 0        -> position 32    : cells 30..34 (d = -2..2)                    -> i0 = 30
+      x = -0.5   -> x*3 = -1.5  -> tie, rounds up to -1/3 -> position 31 2/3: cells 30..34 (29 is 2 2/3 away: outside)     -> i0 = 30
+      x = -0.7   -> x*3 = -2.1  -> nearest third -2/3     -> position 31 1/3: cells 29..33 (29 is 2 1/3 away: inside)      -> i0 = 29
+      x = +0.9   -> x*3 = 2.7   -> nearest third 1        -> position 33    : cells 31..35                                 -> i0 = 31
+    The sub-offset row advances by one per third of a cell and the cell advances when it wraps (R4: q div O, q mod O),
+    so the five samples, which sit at thirds -2, -1, 0, +1, +3 of cell 32, must have rows that differ by exactly those
+    steps modulo 3 with i0 stepping at the wrap.  The absolute phase of the row for odd O*S (which third is row 0) is
+    part of the declared "parity unpinned: physical tap positions" (R8/R24) -- no BASELINE config uses it."""
+    xs = np.array([0.4, 0.0, -0.5, -0.7, 0.9], dtype=np.float32)
+    uvw = np.zeros((len(xs), 3), np.float32)
+    uvw[:, 0] = xs
+    q = oracle_mod.quantise(64, 5, 3, 1, uvw)
+    assert list(q["valid"]) == [1] * 5
+    assert list(q["i0"]) == [30, 30, 30, 29, 31]
+    thirds = np.array([1, 0, -1, -2, 3])                       # snapped position in thirds of a cell from cell 32
+    lin = np.asarray(q["i0"], dtype=np.int64) * 3 + np.asarray(q["su"], dtype=np.int64)     # q of R4
+    assert np.array_equal(lin - lin[1], thirds - thirds[1])   # one row per third, cell carries at the wrap
+    assert all(0 <= r < 3 for r in q["su"])
+    # the v axis runs through the same code path with the same constants
+    uvw2 = np.zeros_like(uvw)
+    uvw2[:, 1] = xs
+    q2 = oracle_mod.quantise(64, 5, 3, 1, uvw2)
+    assert list(q2["j0"]) == [30, 30, 30, 29, 31] and list(q2["sv"]) == list(q["su"])
 
 
 def test_compress_oracle_runs_and_invariance(oracle_mod):

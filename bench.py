@@ -161,14 +161,41 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def ncu_traffic(workload):
+def kernel_source_sha256():
+    """Fingerprint of the gridding kernel's source (the file an ncu capture of the hot kernel depends on)."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in ("grid_warp_kernel.cuh", "grid_kernel.cuh", "gridder_common.cuh"):
+        with open(os.path.join(ROOT, "paper_1605_07023_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, kernel_name):
     """DRAM bytes per launch of the gridding kernel (dram__bytes_read.sum + dram__bytes_write.sum) from
-    the committed `ncu --set full` capture of this workload (profiles/ncu_traffic.json), else None."""
+    the committed `ncu --set full` capture of this workload (profiles/ncu_traffic.json).  The entry is
+    stamped with the kernel's template name and a hash of the kernel sources at capture time; if either
+    differs from what runs now the capture is stale and None is returned instead of an old constant."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+            e = json.load(f).get(workload, {})
     except (OSError, ValueError):
         return None
+    if e.get("kernel") != kernel_name or e.get("source_sha256") != kernel_source_sha256():
+        return None
+    return e.get("dram_bytes_per_launch")
+
+
+def kernel_template_name(info, P, S, op="grid"):
+    """Name of the launched hot kernel as ncu prints it (template arguments from the plan)."""
+    if info["variant"] == 0:
+        return "grid_scatter_kernel<%d>" % P
+    if info["variant"] == 1:
+        return "grid_coarsened_kernel<%d, %d, %d>" % (info["cu"], info["cv"], P)
+    logs = S.bit_length() - 1
+    return "grid_warp_kernel<%d, %d, %d, %d, %d, %d, %d, %d>" % (
+        info["cu"], info["cv"], P, logs, info["pol_split"], 1 if op == "degrid" else 0,
+        info["taps_global"], 1 if op == "dense" else 0)
 
 
 def parse_tuning(text):
@@ -233,8 +260,7 @@ def run_ours(args):
         plan.set_tuning(**tuning)
     plan.allocate_workspace(dev)
     info = plan.info()
-    kernel_name = {0: "grid_scatter_kernel", 1: "grid_coarsened_kernel", 3: "grid_warp_kernel"}[info["variant"]]
-    kernel_name += "<%d,%d,%d>" % (info["cu"], info["cv"], P)
+    kernel_name = kernel_template_name(info, P, S, args.op)
 
     # number of valid samples (for the metric) from the library's own quantise pass
     q = plan.quantise(d_uvw)
@@ -357,7 +383,7 @@ def run_ours(args):
                        "tuning": info, "compressed": compressed, "op": args.op},
             "pct_fp32_roofline": 100.0 * value / world * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / PEAK_FP32_TFLOPS, "traffic": ncu_traffic(cfg.name),
+                         "frac": achieved / PEAK_FP32_TFLOPS, "traffic": ncu_traffic(cfg.name, kernel_name),
                          "kernel": kernel_name, "kernel_ms": kernel_ms,
                          "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (derived; DESIGN.md)"},
             "clocks": clocks, "gpu_launches": launches,

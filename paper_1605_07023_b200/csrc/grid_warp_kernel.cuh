@@ -127,7 +127,7 @@ struct WarpKernelTraits {
     static constexpr int MAX_THREADS = ACC >= 48 ? 512 : (ACC >= 24 ? 768 : 1024);
     // shared memory of one group for a batch of B samples per team
     static constexpr bool W64 = TS == 64;                 // 64-bit moved masks live in a second 16-byte record
-    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return (size_t)TPG * (B + 1) * (16 + (W64 ? 16 : 0) + 8 * P); }   // team stride B + 1 slots: see BP
+    __host__ __device__ static constexpr size_t cooked_bytes(int B) { return ((size_t)TPG * (B + 1) * (16 + (W64 ? 16 : 0) + 8 * P) + 15) & ~(size_t)15; }   // team stride B + 1 slots: see BP
     __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
     __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
     __host__ __device__ static constexpr size_t group_bytes(int B) {
@@ -176,8 +176,8 @@ grid_warp_kernel(const GridParams gp) {
     const int BP = B + 1;
     const int cslots = TPG * BP;
     uint4* crec = reinterpret_cast<uint4*>(gbase);                                       // cooked records
-    float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)cslots * 16);               // cooked vis
-    uint4* cmask = reinterpret_cast<uint4*>(gbase + (size_t)cslots * (16 + 8 * P));      // W64 only
+    uint4* cmask = reinterpret_cast<uint4*>(gbase + (size_t)cslots * 16);                // W64 only (16-byte records first)
+    float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)cslots * (W64 ? 32 : 16)); // cooked vis
     unsigned char* rbase = gbase + T::cooked_bytes(B);
     const size_t rstage = T::raw_bytes(B);
     // raw stage layout: vis [slots][P] float2, rec [slots] 8 B, weights [slots] float

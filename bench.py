@@ -45,6 +45,9 @@ def parse_args():
                     help="compress once outside the timed region (PAPER.md:69, 113) and time grid_execute_compressed; "
                          "the rate then counts compressed samples, as the paper's does")
     ap.add_argument("--tuning", default="", help="e.g. cu=2,cv=2,threads_per_cta=256")
+    ap.add_argument("--no-per-config", action="store_true",
+                    help="skip the per_config table (every BASELINE.json config, device-resident, with an oracle row band)")
+    ap.add_argument("--per-config-steps", type=int, default=5)
     return ap.parse_args()
 
 
@@ -224,6 +227,76 @@ def reduce_over_ranks(times_ms, units, device, world):
     return [float(x) for x in t.tolist()], float(tot.item())
 
 
+ALL_CONFIGS = ["cfg0", "cfg1", "cfg2", "cfg3"] + [f"cfg4_S{s}_P{p}" for s in (4, 8, 16, 32) for p in (1, 4)]
+
+
+def measure_config(name, steps, warmup, dev, oracle_band=True):
+    """One BASELINE.json config, device-resident: K timed grid_execute calls (CUDA events on the launching
+    stream, L2 scrubbed between steps when the inputs could stay in it), the hot kernel's own time, and the
+    rel-L2 / max-abs error of one band of grid rows against the float64 oracle (row-restricted mode)."""
+    import torch
+    from paper_1605_07023_b200 import binding, synth
+    cfg = synth.get_config(name)
+    wl = synth.make_workload(cfg)
+    N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
+    d_uvw, d_vis, d_wts, d_kern = (torch.from_numpy(a).to(dev) for a in (wl.uvw, wl.vis, wl.weights, wl.kernel))
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(cfg.n_vis)
+    plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    plan.allocate_workspace(dev)
+    info = plan.info()
+    q = plan.quantise(d_uvw)
+    n_valid = int(q[:, 5].sum().item())
+    del q
+    updates = n_valid * S * S * P
+    stream = torch.cuda.current_stream()
+    plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)            # the run that is checked against the oracle
+    torch.cuda.synchronize()
+    err = None
+    if oracle_band:
+        import oracle
+        lo = N // 2 + N // 8
+        ref = oracle.grid(N, S, O, W, P, wl.uvw, wl.vis, wl.weights, wl.kernel, rows=(lo, lo + 4))
+        got = grid[lo:lo + 4].cpu().numpy().astype(np.complex128)
+        err = {"rows": [lo, lo + 4], "rel_l2": float(np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel())),
+               "max_abs_over_max": float(np.abs(got - ref).max() / np.abs(ref).max())}
+    for _ in range(max(warmup, 3) - 1):
+        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+    input_bytes = wl.uvw.nbytes + wl.vis.nbytes + wl.weights.nbytes
+    flush_l2 = input_bytes < 2 * 126 * (1 << 20)
+    scrub = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush_l2 else None
+    k_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    s_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in k_ev:
+        a.record(stream)
+        b.record(stream)
+    torch.cuda.synchronize()
+    launches = 0
+    for k in range(steps):
+        plan.set_kernel_events(*k_ev[k])
+        if flush_l2:
+            scrub.fill_(k & 0xff)
+        s_ev[k][0].record(stream)
+        plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        s_ev[k][1].record(stream)
+        launches += plan.last_launches()
+    torch.cuda.synchronize()
+    plan.set_kernel_events(None, None)
+    ms = float(np.mean([a.elapsed_time(b) for a, b in s_ev]))
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
+    plan.destroy()
+    rate = updates / (ms * 1e-3)
+    return {"workload": name, "support": S, "n_pol": P, "grid": N, "n_wplanes": W, "n_vis": cfg.n_vis,
+            "updates_per_step": updates, "steps": steps, "ms_per_step": ms, "value": rate, "unit": "updates/s",
+            "pct_fp32_roofline": 100.0 * rate * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
+            "roofline": {"bound": "alu", "frac": updates * FLOPS_PER_UPDATE / (kernel_ms * 1e-3) / (PEAK_FP32_TFLOPS * 1e12),
+                         "kernel_ms": kernel_ms, "kernel": kernel_template_name(info, P, S)},
+            "block": "%dx%d, pol split %d, %d threads, batch %d" % (info["cu"], info["cv"], info["pol_split"],
+                                                                    info["threads_per_cta"], info["batch"]),
+            "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -398,6 +471,13 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": v, "unit": "updates/s", "cores": cores, "kind": "oracle",
                                     "sample": f"every {stride}th baseline of {cfg.name} ({n_bl} baselines, "
                                               f"{upd:.3e} updates, {dt:.1f} s)"}
+        if (world == 1 and not args.no_per_config and args.op == "grid" and not compressed and not tuning
+                and args.config == "cfg1"):
+            # BASELINE.json's metric is "per config": every config and all 8 points of the config-4 sweep
+            plan.destroy()
+            del d_uvw, d_vis, d_wts, grid, h_uvw, h_vis, h_wts
+            torch.cuda.empty_cache()
+            line["per_config"] = [measure_config(n, args.per_config_steps, 3, dev) for n in ALL_CONFIGS]
         print(json.dumps(line), flush=True)
     plan.destroy()
     if world > 1:

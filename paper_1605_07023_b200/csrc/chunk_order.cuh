@@ -45,8 +45,9 @@ __device__ __forceinline__ long long chunk_first_sample(const GridParams& gp, in
 }
 
 __device__ __forceinline__ uint32_t chunk_tile(const GridParams& gp, int mode, long long c) {
-    const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
-    const uint32_t pos = __ldg(&recs[chunk_first_sample(gp, mode, c)].pos);
+    // records are 8 bytes (CycRec) or, with the weight attached, 16: the origin is the first word either way
+    const uint32_t* words = reinterpret_cast<const uint32_t*>(gp.recs);
+    const uint32_t pos = __ldg(words + (size_t)chunk_first_sample(gp, mode, c) * (gp.rec16 ? 4 : 2));
     const uint32_t tx = (pos & 0x7fffu) >> gp.tile_shift, ty = (pos >> 16) >> gp.tile_shift;
     return ty * 32u + ((ty & 1u) ? 31u - tx : tx);            // boustrophedon over tile rows
 }

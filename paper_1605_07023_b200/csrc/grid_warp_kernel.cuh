@@ -86,13 +86,13 @@ __device__ __forceinline__ uint64_t moved_mask_window128(int from, int to, int l
     return (uint64_t)m;
 }
 
-struct WarpChunk {            // traversal geometry of one chunk (one team), 32 bytes in shared memory
-    long long base;           // mode 0: first position; mode 1: first sample of (baseline, time block)
-    int len;                  // mode 0: positions in the chunk; mode 1: channels in the chunk
-    int h;                    // mode 1: time steps in this block (0: empty chunk)
-    int col0, rowpar;         // mode 0 with layout: column of `base` and parity of its time row;
-                              // mode 1: first channel of the chunk
-    int tile, pad1;           // S = 128: which 64 x 64 tile of the bin this team covers (x + 2 y)
+// Traversal geometry of one chunk (one team): 16 bytes in shared memory, 32-bit sample indices (the callers
+// of this kernel require n_vis < 2^31).
+struct WarpChunk {
+    uint32_t base;            // mode 0: first position; mode 1: first sample of (baseline, time block)
+    uint32_t total;           // positions in the chunk (mode 1: channels x time steps)
+    uint32_t h_col;           // mode 1: time steps of this block | first channel << 16; mode 0 with layout: column of `base`
+    uint32_t flags;           // bit 0: mode 0, parity of the time row of `base`; bits 4-5: tile of a 128 bin (x + 2 y)
 };
 
 __device__ __forceinline__ void cp_async_4(void* dst, const void* src) {
@@ -128,7 +128,7 @@ struct WarpKernelTraits {
     // shared memory of one group for a batch of B samples per team
     static constexpr bool W64 = TS == 64;                 // 64-bit moved masks live in a second 16-byte record
     __host__ __device__ static constexpr size_t cooked_bytes(int B) { return ((size_t)TPG * (B + 1) * (16 + (W64 ? 16 : 0) + 8 * P) + 15) & ~(size_t)15; }   // team stride B + 1 slots: see BP
-    __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (8 + 4 + 8 * P); }
+    __host__ __device__ static constexpr size_t raw_bytes(int B) { return (size_t)TPG * B * (16 + 8 * P); }
     __host__ __device__ static constexpr size_t ctrl_bytes() { return 2 * TPG * sizeof(WarpChunk) + 2 * TPG * 4 + 16; }
     __host__ __device__ static constexpr size_t group_bytes(int B) {
         return (cooked_bytes(B) + 2 * raw_bytes(B) + ctrl_bytes() + 15) & ~(size_t)15;
@@ -180,7 +180,7 @@ grid_warp_kernel(const GridParams gp) {
     float2* cvis = reinterpret_cast<float2*>(gbase + (size_t)cslots * (W64 ? 32 : 16)); // cooked vis
     unsigned char* rbase = gbase + T::cooked_bytes(B);
     const size_t rstage = T::raw_bytes(B);
-    // raw stage layout: vis [slots][P] float2, rec [slots] 8 B, weights [slots] float
+    // raw stage layout: vis [slots][P] float2, then records [slots] {pos, rows, weight, -} of 16 bytes
     WarpChunk* geom = reinterpret_cast<WarpChunk*>(rbase + 2 * rstage);                  // [2][TPG]
     uint32_t* last_pos = reinterpret_cast<uint32_t*>(geom + 2 * TPG);                    // [2][TPG]
     uint32_t* ctrl = last_pos + 2 * TPG;
@@ -222,7 +222,6 @@ grid_warp_kernel(const GridParams gp) {
         my_tu = reinterpret_cast<const unsigned char*>(staps + r0);
         my_tv = reinterpret_cast<const unsigned char*>(staps + s0);
     }
-    const CycRec* recs = reinterpret_cast<const CycRec*>(gp.recs);
 
     float2 acc[CV][CU][PT];
 #pragma unroll
@@ -308,6 +307,10 @@ grid_warp_kernel(const GridParams gp) {
     const int n_batches = mode ? (gp.chunk_cols * gp.tc + B - 1) >> bshift
                                : (gp.chunk + B - 1) >> bshift;
 
+    const uint32_t n_vis32 = (uint32_t)gp.n_vis, n_chan = (uint32_t)gp.n_chan;
+    const uint32_t tc = (uint32_t)gp.tc;               // a power of two (grid_plan_set_traversal)
+    const int tshift = 31 - __clz((int)(tc > 0 ? tc : 1));
+
     // a9: take the next chunk group from the queue; lanes t < TPG work out their team's geometry
     auto fetch = [&](int par) -> long long {
         uint32_t v = 0;
@@ -321,91 +324,99 @@ grid_warp_kernel(const GridParams gp) {
         }
         const long long g = v;
         if (g < n_groups && lg < TPG) {
-            long long chunk_id = (g / NT) * TPG + lg;      // tiled bins: NT consecutive queue entries share a chunk
+            uint32_t chunk_id = (uint32_t)(g / NT) * TPG + lg;      // tiled bins: NT consecutive queue entries share a chunk
             bool have = true;
             if (gp.order) {                            // locality-sorted queue (chunk_order.cuh)
-                have = chunk_id < chunk_count(gp, mode);
+                have = chunk_id < (uint32_t)chunk_count(gp, mode);
                 if (have) chunk_id = __ldg(gp.order + chunk_id);
             }
             WarpChunk cg;
-            cg.base = 0; cg.len = 0; cg.h = 0; cg.col0 = 0; cg.rowpar = 0; cg.tile = (int)(g % NT); cg.pad1 = 0;
+            cg.base = 0; cg.total = 0; cg.h_col = 1; cg.flags = (uint32_t)(g % NT) << 4;
             if (!have) {
             } else if (mode == 0) {
-                cg.base = chunk_id * gp.chunk;
-                const long long left = gp.n_vis - cg.base;
-                cg.len = left <= 0 ? 0 : (left < gp.chunk ? (int)left : gp.chunk);
-                if (gp.n_chan > 0) {
-                    const long long row = cg.base / gp.n_chan;
-                    cg.col0 = (int)(cg.base - row * gp.n_chan);
-                    cg.rowpar = (int)(row & 1);
+                const unsigned long long base = (unsigned long long)chunk_id * (uint32_t)gp.chunk;
+                if (base < n_vis32) {
+                    cg.base = (uint32_t)base;
+                    const uint32_t left = n_vis32 - cg.base;
+                    cg.total = left < (uint32_t)gp.chunk ? left : (uint32_t)gp.chunk;
+                    if (n_chan > 0) {
+                        const uint32_t row = cg.base / n_chan;
+                        cg.h_col = cg.base - row * n_chan;
+                        cg.flags |= row & 1u;
+                    }
                 }
-            } else if (chunk_id < gp.n_chunks_b) {
+            } else if (chunk_id < (uint32_t)gp.n_chunks_b) {
                 // chunk = (baseline, block of tc time steps, block of chunk_cols channels)
-                const long long per_bl = (long long)gp.n_tblocks * gp.n_cblocks;
-                const long long bl = chunk_id / per_bl;
-                const int rem = (int)(chunk_id - bl * per_bl);
-                const int tb = rem / gp.n_cblocks, cc = rem - tb * gp.n_cblocks;
-                cg.h = gp.n_times - tb * gp.tc < gp.tc ? gp.n_times - tb * gp.tc : gp.tc;
-                cg.base = (bl * gp.n_times + (long long)tb * gp.tc) * gp.n_chan;
-                cg.col0 = cc * gp.chunk_cols;
-                cg.len = gp.n_chan - cg.col0 < gp.chunk_cols ? gp.n_chan - cg.col0 : gp.chunk_cols;
+                const uint32_t per_bl = (uint32_t)(gp.n_tblocks * gp.n_cblocks);
+                const uint32_t bl = chunk_id / per_bl, rem = chunk_id - bl * per_bl;
+                const uint32_t tb = rem / (uint32_t)gp.n_cblocks, cc = rem - tb * (uint32_t)gp.n_cblocks;
+                const uint32_t tleft = (uint32_t)gp.n_times - tb * tc;
+                const uint32_t h = tleft < tc ? tleft : tc;
+                const uint32_t col0 = cc * (uint32_t)gp.chunk_cols;
+                const uint32_t cleft = n_chan - col0;
+                cg.base = (bl * (uint32_t)gp.n_times + tb * tc) * n_chan;
+                cg.total = (cleft < (uint32_t)gp.chunk_cols ? cleft : (uint32_t)gp.chunk_cols) * h;
+                cg.h_col = h | (col0 << 16);
             }
-            geom[par * TPG + lg] = cg;
+            *reinterpret_cast<uint4*>(&geom[par * TPG + lg]) = make_uint4(cg.base, cg.total, cg.h_col, cg.flags);
         }
         group_sync();
         return g;
     };
 
     auto count_of = [&](const WarpChunk& cg, int b) -> int {
-        if (mode == 0) {
-            const int left = cg.len - (b << bshift);
-            return left < 0 ? 0 : (left < B ? left : B);
-        }
-        const int left = cg.len * cg.h - (b << bshift);        // columns of h time steps, walked one after another
+        const int left = (int)cg.total - (b << bshift);
         return left < 0 ? 0 : (left < B ? left : B);
     };
 
-    auto sample_of = [&](const WarpChunk& cg, int b, int k) -> long long {
+    // sample (input index) at position q of the chunk's walk
+    auto sample_of = [&](const WarpChunk& cg, int q) -> uint32_t {
         if (mode == 0) {
-            const int off = (b << bshift) + k;
-            long long a = cg.base + off;
-            if (gp.n_chan > 0) {                        // serpentine over time rows
-                const uint32_t col = (uint32_t)(cg.col0 + off);
-                const uint32_t radd = col / (uint32_t)gp.n_chan;
-                const int colr = (int)(col - radd * (uint32_t)gp.n_chan);
-                if ((cg.rowpar + radd) & 1u) a += gp.n_chan - 1 - 2 * colr;
+            uint32_t a = cg.base + (uint32_t)q;
+            if (n_chan > 0) {                          // serpentine over time rows: odd rows are walked backwards
+                uint32_t col = cg.h_col + (uint32_t)q, radd = 0;
+                if (col >= n_chan) {                   // a chunk spans few rows: subtract instead of dividing
+                    col -= n_chan; radd = 1;
+                    if (col >= n_chan) { const uint32_t r2 = col / n_chan; col -= r2 * n_chan; radd += r2; }
+                }
+                if ((cg.flags + radd) & 1u) a += n_chan - 1u - 2u * col;
             }
             return a;
         }
-        const int q = (b << bshift) + k;
-        const int ci = (int)((uint32_t)q / (uint32_t)cg.h), tt = q - ci * cg.h;
-        const int col = cg.col0 + ci;
-        const int ti = (col & 1) ? cg.h - 1 - tt : tt;
-        return cg.base + (long long)ti * gp.n_chan + col;
+        // columns of h time steps, walked one after another, odd columns backwards
+        const uint32_t h = cg.h_col & 0xffffu, col0 = cg.h_col >> 16;
+        uint32_t ci, tt;
+        if (h == tc) { ci = (uint32_t)q >> tshift; tt = (uint32_t)q & (tc - 1u); }
+        else { ci = (uint32_t)q / h; tt = (uint32_t)q - ci * h; }
+        const uint32_t col = col0 + ci;
+        const uint32_t ti = (col & 1u) ? h - 1u - tt : tt;
+        return cg.base + ti * n_chan + col;
     };
 
-    // DEGRID: sample indices are kept as 31-bit offsets from here (a mirrored time row of the
-    // channel-innermost walk reaches back to the start of its row, before the chunk's first position)
-    auto out_base = [&](const WarpChunk& cg) -> long long { return mode == 0 ? cg.base - cg.col0 : cg.base; };
-
-    // a3: start the copies of batch b of the chunk group `par` into raw stage `st`
+    // a3: start the copies of batch b of the chunk group `par` into raw stage `st`: per sample one 16-byte
+    // record {origin, tap rows, weight} (8 bytes + a separate weight for pre-quantised, compressed input)
+    // and its visibilities
     auto issue = [&](int par, int b, int st) {
         unsigned char* rs = rbase + (size_t)st * rstage;
         float2* rvis = reinterpret_cast<float2*>(rs);
-        CycRec* rrec = reinterpret_cast<CycRec*>(rs + (size_t)slots * 8 * P);
-        float* rw = reinterpret_cast<float*>(rs + (size_t)slots * (8 * P + 8));
+        uint4* rrec = reinterpret_cast<uint4*>(rs + (size_t)slots * 8 * P);
         for (int kk = lg; kk < slots; kk += GT) {
             const int t = kk >> bshift, k = kk & (B - 1);
-            const WarpChunk cg = geom[par * TPG + t];
+            const uint4 g4 = *reinterpret_cast<const uint4*>(&geom[par * TPG + t]);
+            const WarpChunk cg = {g4.x, g4.y, g4.z, g4.w};
             if (k >= count_of(cg, b)) continue;
-            const long long g = sample_of(cg, b, k);
-            cp_async_8(rrec + kk, recs + g);
-            if (gp.weights) cp_async_4(rw + kk, gp.weights + g);       // null: pre-weighted (compressed) input
+            const uint32_t g = sample_of(cg, (b << bshift) + k);
+            if (gp.rec16) {
+                cp_async_16(rrec + kk, reinterpret_cast<const uint4*>(gp.recs) + g);
+            } else {
+                cp_async_8(rrec + kk, reinterpret_cast<const CycRec*>(gp.recs) + g);
+                if (gp.weights) cp_async_4(&rrec[kk].z, gp.weights + g);   // null: pre-weighted (compressed) input
+            }
             if constexpr (DEGRID) {
             } else if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
             else {
 #pragma unroll
-                for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + g * P + q);
+                for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + (size_t)g * P + q);
             }
         }
         cp_async_commit();
@@ -415,66 +426,74 @@ grid_warp_kernel(const GridParams gp) {
     auto cook = [&](int par, int b, int st) {
         const unsigned char* rs = rbase + (size_t)st * rstage;
         const float2* rvis = reinterpret_cast<const float2*>(rs);
-        const CycRec* rrec = reinterpret_cast<const CycRec*>(rs + (size_t)slots * 8 * P);
-        const float* rw = reinterpret_cast<const float*>(rs + (size_t)slots * (8 * P + 8));
+        const uint4* rrec = reinterpret_cast<const uint4*>(rs + (size_t)slots * 8 * P);
+        const bool unit_w = !gp.rec16 && !gp.weights;
         for (int kk = lg; kk < slots; kk += GT) {
             const int t = kk >> bshift, k = kk & (B - 1);
-            const WarpChunk cg = geom[par * TPG + t];
+            const uint4 g4 = *reinterpret_cast<const uint4*>(&geom[par * TPG + t]);
+            const WarpChunk cg = {g4.x, g4.y, g4.z, g4.w};
             const int cnt = count_of(cg, b);
+            const int ck = t * BP + k;                 // slot in the cooked arrays
             uint4 c = make_uint4(0u, 0u, 0u, 0u);
+            if constexpr (W64) cmask[ck] = make_uint4(0u, 0u, 0u, 0u);
+            uint32_t code = 0xffffffffu;               // DEGRID: where the result goes; all ones = no sample
             float w = 0.f;
             bool valid = false;
-            const int ck = t * BP + k;                 // slot in the cooked arrays
-            if constexpr (W64) cmask[ck] = make_uint4(0u, 0u, 0u, 0u);
             if (k < cnt) {
-                const CycRec rec = rrec[kk];
+                const uint4 rec = rrec[kk];
                 mask_t mx = 0, my = 0;
                 if (k > 0 || b > 0) {
-                    const uint32_t pp = k > 0 ? rrec[kk - 1].pos : last_pos[((b - 1) & 1) * TPG + t];
+                    const uint32_t pp = k > 0 ? rrec[kk - 1].x : last_pos[((b - 1) & 1) * TPG + t];
+                    const int tile = (int)((cg.flags >> 4) & 3u);
                     if constexpr (NT > 1) {
-                        mx = moved_mask_window128((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu), (cg.tile & 1) * TS);
-                        my = moved_mask_window128((int)(pp >> 16), (int)(rec.pos >> 16), (cg.tile >> 1) * TS);
+                        mx = moved_mask_window128((int)(pp & 0x7fffu), (int)(rec.x & 0x7fffu), (tile & 1) * TS);
+                        my = moved_mask_window128((int)(pp >> 16), (int)(rec.x >> 16), (tile >> 1) * TS);
                     } else if constexpr (W64) {
-                        mx = moved_mask64((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
-                        my = moved_mask64((int)(pp >> 16), (int)(rec.pos >> 16));
+                        mx = moved_mask64((int)(pp & 0x7fffu), (int)(rec.x & 0x7fffu));
+                        my = moved_mask64((int)(pp >> 16), (int)(rec.x >> 16));
                     } else {
-                        mx = moved_mask<LOGS>((int)(pp & 0x7fffu), (int)(rec.pos & 0x7fffu));
-                        my = moved_mask<LOGS>((int)(pp >> 16), (int)(rec.pos >> 16));
+                        mx = moved_mask<LOGS>((int)(pp & 0x7fffu), (int)(rec.x & 0x7fffu));
+                        my = moved_mask<LOGS>((int)(pp >> 16), (int)(rec.x >> 16));
                     }
                 }
-                if (k == cnt - 1) last_pos[(b & 1) * TPG + t] = rec.pos;
-                const int i0 = (int)(rec.pos & 0x7fffu), j0 = (int)(rec.pos >> 16);
-                const uint32_t xo = (rec.rows & 0xffffu) * ROW + S - (i0 & (S - 1));
-                const uint32_t yo = (rec.rows >> 16) * ROW + S - (j0 & (S - 1));
-                c.x = rec.pos & 0xffff7fffu;
+                if (k == cnt - 1) last_pos[(b & 1) * TPG + t] = rec.x;
+                const int i0 = (int)(rec.x & 0x7fffu), j0 = (int)(rec.x >> 16);
+                const uint32_t xo = (rec.y & 0xffffu) * ROW + S - (i0 & (S - 1));
+                const uint32_t yo = (rec.y >> 16) * ROW + S - (j0 & (S - 1));
+                c.x = rec.x & 0xffff7fffu;
                 if constexpr (DENSE) {
                     // table row ((wp*O + sv)*O + su), in elements of S*S
-                    const uint32_t ru = rec.rows & 0xffffu, rv = rec.rows >> 16;
+                    const uint32_t ru = rec.y & 0xffffu, rv = rec.y >> 16;
                     const uint32_t su = ru - (ru / (uint32_t)gp.oversample) * (uint32_t)gp.oversample;
                     c.y = (rv * (uint32_t)gp.oversample + su) * (uint32_t)(S * S);
                     c.z = mx; c.w = my;
                 } else if constexpr (W64) {
-                    c.y = rec.rows;
+                    c.y = rec.y;
                     cmask[ck] = make_uint4((uint32_t)mx, (uint32_t)((uint64_t)mx >> 32), (uint32_t)my, (uint32_t)((uint64_t)my >> 32));
                 }
-                else if constexpr (WIDE && TG) { c.y = rec.rows; c.z = mx; c.w = my; }     // offsets exceed 16 bits
+                else if constexpr (WIDE && TG) { c.y = rec.y; c.z = mx; c.w = my; }     // offsets exceed 16 bits
                 else if constexpr (WIDE) { c.y = xo | (yo << 16); c.z = mx; c.w = my; }
                 else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
-                valid = (rec.pos & 0x8000u) == 0;
-                if (valid) w = gp.weights ? rw[kk] : 1.f;
+                valid = (rec.x & 0x8000u) == 0;
+                if (valid) w = unit_w ? 1.f : __uint_as_float(rec.z);
+                if constexpr (DEGRID) code = sample_of(cg, (b << bshift) + k) | (valid ? 0u : 0x80000000u);
             }
             crec[ck] = c;
             if constexpr (DEGRID) {
-                // where the result goes: offset from the chunk base, bit 31 = skipped sample, all ones = no sample
-                uint32_t code = 0xffffffffu;
-                if (k < cnt) code = (uint32_t)(sample_of(cg, b, k) - out_base(cg)) | (valid ? 0u : 0x80000000u);
                 cvis[(size_t)ck * P] = make_float2(w, __uint_as_float(code));
+            } else if constexpr (P == 1) {
+                float2 v = make_float2(0.f, 0.f);
+                if (valid) { v = rvis[kk]; v.x *= w; v.y *= w; }        // skipped: exact zeros, whatever the input holds
+                cvis[ck] = v;
             } else {
+                // pre-weighting, 16 bytes at a time
+                const float4* src = reinterpret_cast<const float4*>(rvis + (size_t)kk * P);
+                float4* dst = reinterpret_cast<float4*>(cvis + (size_t)ck * P);
 #pragma unroll
-                for (int q = 0; q < P; ++q) {
-                    float2 v = make_float2(0.f, 0.f);
-                    if (valid) { v = rvis[(size_t)kk * P + q]; v.x *= w; v.y *= w; }
-                    cvis[(size_t)ck * P + q] = v;
+                for (int q = 0; q < P / 2; ++q) {
+                    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (valid) { v = src[q]; v.x *= w; v.y *= w; v.z *= w; v.w *= w; }
+                    dst[q] = v;
                 }
             }
         }
@@ -485,9 +504,11 @@ grid_warp_kernel(const GridParams gp) {
     if (cur < n_groups) issue(par, 0, 0);
     int st = 0;                                        // raw stage holding the next batch to cook
     while (cur < n_groups) {
-        const WarpChunk my_cg = geom[par * TPG + tg];
+        const uint4 my_g4 = *reinterpret_cast<const uint4*>(&geom[par * TPG + tg]);
+        const WarpChunk my_cg = {my_g4.x, my_g4.y, my_g4.z, my_g4.w};
+        const int my_tile = (int)((my_cg.flags >> 4) & 3u);
         // first owned column / row position (inside my tile of the bin when the bin is tiled)
-        const int px0 = r0 + (NT > 1 ? (my_cg.tile & 1) * TS : 0), py0 = s0 + (NT > 1 ? (my_cg.tile >> 1) * TS : 0);
+        const int px0 = r0 + (NT > 1 ? (my_tile & 1) * TS : 0), py0 = s0 + (NT > 1 ? (my_tile >> 1) * TS : 0);
         bool live = false;
         long long next = cur;
         int next_par = par;
@@ -693,7 +714,7 @@ grid_warp_kernel(const GridParams gp) {
                     constexpr int WLAST = (W0 >> LOGT) > 1 ? (W0 >> LOGT) : 1;      // floats left per lane
                     const uint32_t code = __float_as_uint(meta.y);
                     if ((lt & dup & 31) == 0 && code != 0xffffffffu) {
-                        float* o = reinterpret_cast<float*>(gp.vis_out + (out_base(my_cg) + (long long)(code & 0x7fffffffu)) * P) + first;
+                        float* o = reinterpret_cast<float*>(gp.vis_out + (size_t)(code & 0x7fffffffu) * P) + first;
                         const float w = meta.x;
                         if constexpr (GW > 1 || NT > 1) {
                             // the team spans several warps (and, at S = 128, four tiles in other groups): every

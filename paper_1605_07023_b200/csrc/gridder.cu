@@ -403,7 +403,7 @@ long long ctas_hint(const grid_plan* p) { return (long long)p->n_sm * (p->groups
 
 QuantParams quant_params(const grid_plan* p) {
     QuantParams q;
-    q.format = p->variant == 3 ? 1 : 0;
+    q.format = p->variant == 3 ? 2 : 0;
     q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
     q.oversample = p->O;
     q.shift = p->O - (p->O * p->S + 1) / 2;
@@ -596,6 +596,8 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     const int n_chan = have_layout ? plan->n_channels : 0, n_times = have_layout ? plan->n_times : 0;
     float* hop_stats = reinterpret_cast<float*>(counters + 2);
 
+    if (plan->variant == 3 && n_vis >= 0x7fffffffLL)
+        return fail(GRID_ERR_UNSUPPORTED, "grid_execute: the warp kernel indexes samples with 31 bits (n_vis = %lld)", n_vis);
     // reset the chunk queue and the hop statistics, then a1: quantise pass
     if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
@@ -603,7 +605,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         const long long threads = (n_vis + 3) / 4;
         const long long blocks = (threads + 255) / 256;
         quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, n_vis, quant_params(plan), hop_stats,
-                                                             n_chan, n_times, (float)(plan->bin_u + plan->bin_v));
+                                                             n_chan, n_times, (float)(plan->bin_u + plan->bin_v), weights);
         plan->last_launches++;
     }
 
@@ -616,6 +618,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.grid = grid;
     gp.vis_out = reinterpret_cast<float2*>(degrid_out);
     gp.counters = counters;
+    gp.rec16 = (plan->variant == 3 && !ext_recs) ? 1 : 0;
     gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
     gp.oversample = plan->O;
@@ -779,8 +782,10 @@ int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const flo
     uint32_t* block_counts = reinterpret_cast<uint32_t*>(rbase + (size_t)((n + 3) / 4 * 4) * sizeof(CycRec));   // ... the rest of the 16 B
     if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_compress: %s", cudaGetErrorString(cudaGetLastError()));
+    QuantParams qp = quant_params(plan);
+    qp.format = 1;                                   // compact 8-byte records: what compression compares and emits
     quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
-        uvw, reinterpret_cast<SampleRec*>(recs), n, quant_params(plan), reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
+        uvw, reinterpret_cast<SampleRec*>(recs), n, qp, reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
     compress_count_kernel<<<(unsigned)nb, kCompressBlock, 0, stream>>>(recs, n, block_counts);
     compress_scan_kernel<<<1, 1024, 0, stream>>>(block_counts, (int)nb, out_count);
     const float2* v2 = reinterpret_cast<const float2*>(vis);

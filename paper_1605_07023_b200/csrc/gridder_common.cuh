@@ -22,7 +22,7 @@ static constexpr uint32_t kInvalidRec = 0xFFFFFFFFu;
 struct CycRec { uint32_t pos, rows; };
 
 struct QuantParams {
-    int format;           // 0: SampleRec (16 B), 1: CycRec (8 B)
+    int format;           // 0: SampleRec (16 B), 1: CycRec (8 B), 2: CycRec + weight (16 B: pos, rows, weight, 0)
     double c_centre;      // O*floor(N/2) + 0.5
     int oversample;       // O
     int shift;            // O - ceil(O*S/2)
@@ -56,6 +56,7 @@ struct GridParams {
     int n_cblocks, chunk_cols;   // variant 3, time-innermost: a chunk spans chunk_cols channels
     int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
     float fzero;              // 0.0f the compiler cannot see: accumulators are cleared by moves from the constant bank
+    int rec16;                // warp kernel: records are 16 bytes {pos, rows, weight, -} (quantise format 2), else CycRec
 };
 
 }  // namespace gridb200

@@ -63,7 +63,8 @@ __device__ __forceinline__ SampleRec make_record(const QuantOut& q, const QuantP
 // kernel can walk each chunk along the slower axis (hop_stats[0] channel, [1] time; capped per hop).
 __global__ void __launch_bounds__(256)
 quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, long long n,
-                QuantParams qp, float* __restrict__ hop_stats, int n_chan, int n_times, float hop_cap) {
+                QuantParams qp, float* __restrict__ hop_stats, int n_chan, int n_times, float hop_cap,
+                const float* __restrict__ weights = nullptr) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long first = g * 4;
     if (n_chan > 0 && (blockIdx.x & 63) == 0) {
@@ -98,6 +99,25 @@ quantise_kernel(const float* __restrict__ uvw, SampleRec* __restrict__ recs, lon
         c[7] = b.w; c[8] = d.x; c[9] = d.y; c[10] = d.z; c[11] = d.w;
     } else {
         for (int k = 0; k < 12; ++k) c[k] = (first * 3 + k < n * 3) ? __ldg(uvw + first * 3 + k) : 0.f;
+    }
+    if (qp.format == 2) {                            // the warp kernel's records: the weight travels with the sample
+        float w[4] = {1.f, 1.f, 1.f, 1.f};
+        if (weights) {
+            if (first + 4 <= n) {
+                const float4 w4 = __ldg(reinterpret_cast<const float4*>(weights + first));
+                w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
+            } else {
+                for (int k = 0; k < 4; ++k) if (first + k < n) w[k] = __ldg(weights + first + k);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (first + k < n) {
+                const CycRec r = make_cyc_record(quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp), qp);
+                recs[first + k] = make_uint4(r.pos, r.rows, __float_as_uint(w[k]), 0u);
+            }
+        }
+        return;
     }
     if (qp.format == 1 && first + 4 <= n) {          // four 8-byte records = two 16-byte stores
         CycRec r[4];

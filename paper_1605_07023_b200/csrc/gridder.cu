@@ -101,7 +101,21 @@ WarpDesc pick_warp(int logs) {
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
-WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps) {
+// Row-skip instantiations (grids far beyond the L2: DRAM-bound atomics), for the blocks such plans default to.
+template <int CU, int CV, int P, int PS>
+WarpDesc pick_warp_rs(int logs) {
+#define RSCASE(l) case l: { using T = WarpKernelTraits<CU, CV, P, l, PS>; \
+        return WarpDesc{grid_warp_kernel<CU, CV, P, l, PS, false, false, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; }
+    switch (logs) { RSCASE(2) RSCASE(3) RSCASE(4) }
+#undef RSCASE
+    return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+}
+
+WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps, bool row_skip = false) {
+    if (row_skip) {
+        if (cu == 2 && cv == 2 && P == 4 && ps == 2) { const WarpDesc d = pick_warp_rs<2, 2, 4, 2>(logs); if (d.fn) return d; }
+        if (cu == 2 && cv == 2 && P == 4 && ps == 1) { const WarpDesc d = pick_warp_rs<2, 2, 4, 1>(logs); if (d.fn) return d; }
+    }
 #define CASE(a, b, p, s) if (cu == a && cv == b && P == p && ps == s) return pick_warp<a, b, p, s>(logs);
     CASE(1, 1, 1, 1) CASE(2, 1, 1, 1) CASE(2, 2, 1, 1) CASE(4, 2, 1, 1) CASE(4, 4, 1, 1) CASE(8, 4, 1, 1)
     CASE(1, 1, 2, 1) CASE(2, 2, 2, 1) CASE(4, 2, 2, 1) CASE(4, 4, 2, 1)
@@ -705,7 +719,8 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         kernel_fn fn = plan->dense ? lookup_warp_dense(plan->cu, plan->cv, plan->P, logs).fn
                      : degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs, plan->taps_global != 0)
                      : (plan->variant == 3 && plan->taps_global) ? lookup_warp_tg(plan->cu, plan->cv, plan->P, logs).fn
-                     : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split).fn
+                     : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split,
+                                                        (size_t)plan->N * plan->N * plan->P * sizeof(float2) > ((size_t)1 << 30)).fn
                                           : lookup_kernel(plan->cu, plan->cv, plan->P);
         // a9 locality: sort the chunk ids by grid tile when the grid does not fit the L2
         if (plan->variant == 3) {

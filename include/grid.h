@@ -81,7 +81,9 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
  *   out_records  [>= n_vis] 8-byte records (opaque: cell, sub-offsets, plane), DEVICE, 16-byte aligned
  *   out_vis      [>= n_vis][n_pol] complex64: sum over the run of weights * vis (FP32, input order)
  *   out_count    DEVICE long long: number of compressed samples written
- * Needs the plan's workspace.  Power-of-two supports only (GRID_ERR_UNSUPPORTED otherwise). */
+ * Needs the plan's workspace.  Supports 3..128 on grids of at least twice the padded support (the plans that run
+ * the warp kernel, variant 3); GRID_ERR_UNSUPPORTED otherwise.  For supports that are not powers of two the
+ * records are in the padded form described under grid_plan_set_tuning. */
 int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                   void* out_records, float* out_vis, long long* out_count, grid_stream_t stream);
 
@@ -98,7 +100,7 @@ int grid_execute_compressed(grid_plan* plan, const void* records, const float* v
  *   conv_kernel_2d  [n_wplanes][oversample][oversample][support][support] complex64, DEVICE
  * Everything else as grid_execute (same Q, W, skipping rule, accumulation).  Power-of-two supports up to
  * 32 run on the coarsened kernel with the table read through L1/L2; other supports on a
- * one-atomic-per-update kernel. */
+ * one-atomic-per-update kernel (grid_last_error() says so after the call). */
 int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                        const float* conv_kernel_2d, float* grid, grid_stream_t stream);
 
@@ -107,8 +109,9 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
  *     vis_out[n][p] = weights[n] * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * grid[j0+tj][i0+ti][p]
  * with the same Q, W as grid_execute; skipped samples (R7) get zeros.  <grid_execute(V), G> equals
  * <V, grid_degrid(G)> (pin P7).  grid is read-only; vis_out [n_vis][n_pol] complex64 is overwritten.
- * Two kernels: for power-of-two supports up to 128 the coarsened kernel run backwards -- owned grid values stay in registers while the footprint covers them; otherwise (any
- * support) a gather kernel bound by L2 bandwidth.  grid_plan_set_degrid_gather(plan, 1) forces the latter. */
+ * Two kernels: for supports 3..128 the coarsened kernel run backwards -- owned grid values stay in registers
+ * while the footprint covers them; otherwise (any support) a gather kernel bound by L2 bandwidth.
+ * grid_plan_set_degrid_gather(plan, 1) forces the latter. */
 int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const float* conv_kernel,
                 const float* grid, float* vis_out, grid_stream_t stream);
 
@@ -120,10 +123,17 @@ int grid_plan_set_degrid_gather(grid_plan* plan, int on);
  * Runs the same device function grid_execute uses.  n need not equal the plan's n_vis. */
 int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid_stream_t stream);
 
-/* Override the tuned launch configuration (autotuning).  Any argument <= 0 keeps the
- * current value.  variant: 3 = warp-autonomous coarsened kernel with bin == support (power-of-two
- * supports 4..128; default for those), 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any
- * support; default otherwise), 0 = naive scatter (one atomic per update; diagnostic baseline only).
+/* Override the tuned launch configuration (autotuning).  variant < 0 keeps the current kernel,
+ * any other argument <= 0 keeps its current value (when the variant changes, threads_per_cta and ctas_per_sm fall
+ * back to that variant's defaults unless given).
+ * variant: 3 = warp-autonomous coarsened kernel with bin == support (default for supports 3..128 on grids of at
+ *   least twice the padded support).  Supports that are not powers of two are zero-padded to the next power of
+ *   two Sk (pin P14): every tap row exists in two copies, zeros behind the taps (footprint
+ *   origin unchanged) and zeros in front (origin moved down by Sk - S), the second used only where the padded
+ *   footprint would leave the grid; the result is the same sum, (Sk/S)^2 times the multiply-adds;
+ * 1 = coarsened kernel with the paper's block-aligned, zero-padded bin (any support that fits a CTA; default for
+ *   supports 1, 2 and for tiny grids);
+ * 0 = naive scatter (one atomic per update; diagnostic baseline; never a default for supports 3..128).
  *   cu, cv            coarsening block per thread (u, v), each in {1,2,4,8}, cu*cv*n_pol <= 32
  *   threads_per_cta   multiple of 32, <= 1024
  *   batch             samples staged to shared memory per team per step
@@ -147,7 +157,7 @@ int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block);
  * result is the same sum): 1 = sorted by the coarse grid tile of the chunk's first sample, so that
  * chunks in flight together flush to neighbouring grid cells (three extra small launches per
  * grid_execute), 0 = input (baseline) order, -1 = sorted only when the grid exceeds 256 MB, i.e. twice
- * the L2 (default).  Power-of-two supports (variant 3) only; ignored otherwise. */
+ * the L2 (default).  Variant 3 only; ignored otherwise. */
 int grid_plan_set_chunk_order(grid_plan* plan, int mode);
 
 /* Variant 3, n_pol = 4: spread the polarisations of one grid point over `lanes` adjacent threads

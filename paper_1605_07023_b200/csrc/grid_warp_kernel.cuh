@@ -48,14 +48,23 @@ __device__ __forceinline__ uint32_t moved_mask(int from, int to) {
     return m & ALL;
 }
 
+// Tap t (< Sk) of row `row` of the table the kernel works with.  Supports that are not powers of two are
+// zero-padded to Sk = S + pad: every row of the caller's table appears twice, copy 0 with the zeros behind the S
+// taps, copy 1 with the zeros in front (gridder.cu, padded_support).
+__device__ __forceinline__ float2 padded_tap(const float2* __restrict__ kern, long long row, int t, int S_real, int pad) {
+    if (pad == 0) return __ldg(kern + row * S_real + t);
+    const int src = (row & 1) ? t - pad : t;
+    return (src >= 0 && src < S_real) ? __ldg(kern + (row >> 1) * S_real + src) : make_float2(0.f, 0.f);
+}
+
 // Row-doubled copy of the tap table in global memory (TG kernels): t[r][k] = kern[r][k mod S], k < 2S.
 __global__ void __launch_bounds__(256) tap_table_kernel(const float2* __restrict__ kern, float2* __restrict__ out,
-                                                        long long n_elems, int S) {
+                                                        long long n_elems, int S, int pad) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_elems) return;
     const long long r = k / (2 * S);
     const int t = (int)(k - r * 2 * S) & (S - 1);
-    out[k] = __ldg(kern + r * S + t);
+    out[k] = padded_tap(kern, r, t, S - pad, pad);
 }
 
 // The same for a 64-wide bin (S = 64): 64-bit mask.
@@ -189,7 +198,7 @@ grid_warp_kernel(const GridParams gp) {
     if constexpr (!TG && !DENSE) {
         for (int k = tid; k < gp.n_rows * ROW; k += blockDim.x) {      // a4
             const int r = k / ROW, t = (k - r * ROW) & (S - 1);
-            staps[k] = __ldg(gp.kern + (size_t)r * S + t);
+            staps[k] = padded_tap(gp.kern, r, t, S - gp.tap_pad, gp.tap_pad);
         }
     }
     __syncthreads();

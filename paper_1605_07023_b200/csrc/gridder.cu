@@ -34,6 +34,7 @@ int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 struct grid_plan {
     int N, S, O, W, P;
+    int Sk;                               // support the warp kernel runs with: S, or the next power of two (zero-padded taps)
     long long n_vis;
     int n_baselines, n_times, n_channels;
     void* workspace;
@@ -51,6 +52,7 @@ struct grid_plan {
     int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on      // variant 3: warp groups per CTA; teams per queue entry (all variants)
     int n_sm, max_smem;
     int last_launches;
+    int user_tuned;                       // set_tuning / set_pol_split was called: set_samples keeps the block
     cudaEvent_t ev_start, ev_stop;
 };
 
@@ -228,13 +230,33 @@ int log2_exact(int v) {
     return -1;
 }
 
+// Supports that are not powers of two run on the warp kernel with the tap rows zero-padded to the next power
+// of two (pin P14: zero taps leave the grid unchanged).  Two padded copies of every row:
+// zeros behind the taps (footprint origin unchanged), and zeros in front (origin moved down by the padding) for
+// samples whose padded footprint would otherwise stick out of the grid's upper edge -- so the kernel needs no
+// bounds test.  Needs N >= 2*Sk - S (a footprint cannot touch both edges).
+int padded_support(int S, int N, int W, int O) {
+    if (S < 3 || S > 128) return S;
+    int sk = 4;
+    while (sk < S) sk *= 2;
+    if (sk == S) return S;
+    if (N < 2 * sk - S || (long long)W * O * 2 > 65535) return S;
+    return sk;
+}
+bool is_padded(const grid_plan* p) { return p->Sk != p->S; }
+int tap_rows(const grid_plan* p) { return p->W * p->O * (is_padded(p) ? 2 : 1); }
+
 size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec); }
 
 // workspace: [256 B counters][order bins][records][chunk order]
 constexpr size_t kHeadBytes = 256 + 2 * kOrderBins * sizeof(uint32_t);
 size_t order_capacity(const grid_plan* p) { return (size_t)(p->n_vis / 8 + 4096); }
+size_t tap_table_bytes(const grid_plan* p);
+size_t tap_table_offset(const grid_plan* p) {
+    return kHeadBytes + records_bytes(p) + ((order_capacity(p) * sizeof(uint32_t) + 15) & ~(size_t)15);
+}
 size_t tap_table_bytes(const grid_plan* p) {
-    return p->taps_global ? (size_t)p->W * p->O * 2 * p->S * sizeof(float2) : 0;
+    return p->taps_global ? (size_t)tap_rows(p) * 2 * p->Sk * sizeof(float2) : 0;
 }
 
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
@@ -248,9 +270,10 @@ int derive(grid_plan* p) {
     }
     p->groups_per_cta = 0;
     if (p->variant == 3) {
-        const int logs = log2_exact(p->S);
+        const int logs = log2_exact(p->Sk);
         if (logs < 2 || logs > 7)
-            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a power-of-two support in [4, 128], got %d", p->S);
+            return fail(GRID_ERR_UNSUPPORTED, "variant 3 needs a support in [3, 128] (padded to a power of two) and a grid of "
+                        "at least twice the padded support, got support %d on a grid of %d", p->S, p->N);
         WarpDesc d = lookup_warp(p->cu, p->cv, p->P, logs, p->pol_split);
         if (!d.fn)
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
@@ -263,11 +286,11 @@ int derive(grid_plan* p) {
         }
         // Tap table: in shared memory when it leaves at least half of it to the warp groups (and, for S = 32,
         // its offsets fit the record's 16 bits); otherwise read through L1/L2 from global memory (TG kernels).
-        size_t taps = ((size_t)p->W * p->O * 2 * p->S * sizeof(float2) + 15) & ~(size_t)15;
+        size_t taps = ((size_t)tap_rows(p) * 2 * p->Sk * sizeof(float2) + 15) & ~(size_t)15;
         p->taps_global = 0;
         if (p->dense) taps = 0;
         else if (taps > (size_t)p->max_smem / 2 || taps + d.group_bytes(p->batch) > (size_t)p->max_smem ||
-            (logs == 5 && (long long)p->W * p->O * 2 * p->S > 65535)) {
+            (logs == 5 && (long long)tap_rows(p) * 2 * p->Sk > 65535)) {
             const WarpDesc g = p->pol_split == 1 ? lookup_warp_tg(p->cu, p->cv, p->P, logs) : WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
             if (!g.fn)
                 return fail(GRID_ERR_UNSUPPORTED, "tap table (%zu B) needs the global-memory kernels, which are instantiated "
@@ -285,10 +308,10 @@ int derive(grid_plan* p) {
         int threads = p->threads < d.max_threads ? p->threads : d.max_threads;
         if (threads < d.gt)
             return fail(GRID_ERR_UNSUPPORTED, "a bin needs %d threads but the CTA may have %d", d.gt, threads);
-        p->bin_u = p->bin_v = p->S;
-        p->row_u = p->row_v = 2 * p->S;
-        p->nbx = (p->S > 64 ? 64 : p->S) / p->cu;          // S = 128: a team covers a 64 x 64 tile of the bin
-        p->nby = (p->S > 64 ? 64 : p->S) / p->cv;
+        p->bin_u = p->bin_v = p->Sk;
+        p->row_u = p->row_v = 2 * p->Sk;
+        p->nbx = (p->Sk > 64 ? 64 : p->Sk) / p->cu;        // S = 128: a team covers a 64 x 64 tile of the bin
+        p->nby = (p->Sk > 64 ? 64 : p->Sk) / p->cv;
         p->team_threads = d.team;
         int groups = threads / d.gt;
         if (d.gt > 32 && groups > 15) groups = 15;                 // one named barrier per group
@@ -366,7 +389,7 @@ void default_tuning(grid_plan* p) {
     }
     if (p->S < 4) { p->cu = 1; p->cv = 1; }
     // power-of-two supports: bin == support, no padding (grid_warp_kernel.cuh)
-    const int logs = log2_exact(p->S);
+    const int logs = log2_exact(p->Sk);
     if (logs >= 2 && logs <= 7) {
         grid_plan trial = *p;
         trial.variant = 3;
@@ -386,6 +409,10 @@ void default_tuning(grid_plan* p) {
         else if (logs == 2) { trial.cu = 2; trial.cv = 2; }
         else if (logs >= 5) { trial.cu = 8; trial.cv = 4; }
         else { trial.cu = 4; trial.cv = 4; }
+        // Small inputs (fewer than ~4096 samples per SM; "low occupancy ... when the data is sparse") are
+        // bound by the latency of a team's sequential walk, not by issue slots: small blocks spread a bin over more
+        // threads (cfg0: 2x2 runs in 0.025 ms where 4x4 needs 0.054 ms).
+        if (trial.n_vis >= 0 && trial.n_vis < 4096LL * trial.n_sm && logs <= 4) { trial.cu = 2; trial.cv = 2; }
         // several teams share a warp at small supports: shrink the batch until all warps fit
         while (trial.batch > 8) {
             grid_plan probe = trial;
@@ -398,6 +425,7 @@ void default_tuning(grid_plan* p) {
         // tap table beyond shared memory: the global-memory kernels exist for split 1 and the default blocks
         trial.pol_split = 1;
         if (trial.P >= 4 && logs == 4) { trial.cu = 4; trial.cv = 2; }
+        if (trial.P == 2) { trial.cu = 4; trial.cv = 2; }
         trial.batch = 32;
         if (derive(&trial) == GRID_OK) { *p = trial; return; }
     }
@@ -408,8 +436,13 @@ void default_tuning(grid_plan* p) {
         // and as the last resort the one-atomic-per-update kernel, which handles any support
         const int tries[4][2] = {{4, 2}, {2, 2}, {2, 1}, {1, 1}};
         for (int t = 0; t < 4 && derive(p) != GRID_OK; ++t) { p->cu = tries[t][0]; p->cv = tries[t][1]; p->threads = 512; }
-        if (derive(p) != GRID_OK) { p->variant = 0; p->cu = p->cv = 1; }
-        g_err[0] = 0;
+        if (derive(p) != GRID_OK) {
+            p->variant = 0; p->cu = p->cv = 1;
+            snprintf(g_err, sizeof(g_err), "note: support %d on a grid of %d has no coarsened kernel; this plan uses the "
+                     "one-atomic-per-update kernel (correct, slow)", p->S, p->N);
+        } else {
+            g_err[0] = 0;
+        }
     }
 }
 
@@ -423,6 +456,9 @@ QuantParams quant_params(const grid_plan* p) {
     q.shift = p->O - (p->O * p->S + 1) / 2;
     q.q_limit = (p->N - p->S + 1) * p->O;
     q.n_wplanes = p->W;
+    q.pad = (p->variant == 3 && is_padded(p)) ? p->Sk - p->S : 0;
+    q.sk = p->Sk;
+    q.grid_size = p->N;
     const bool scatter = p->variant == 0;
     q.cu = scatter ? 1 : p->cu;
     q.cv = scatter ? 1 : p->cv;
@@ -468,6 +504,7 @@ grid_plan* grid_plan_create(int grid_size, int support, int oversample, int n_wp
     if (!p) { fail(GRID_ERR_INVALID_ARG, "out of host memory"); return nullptr; }
     memset(p, 0, sizeof(*p));
     p->N = grid_size; p->S = support; p->O = oversample; p->W = n_wplanes; p->P = n_pol;
+    p->Sk = padded_support(support, grid_size, n_wplanes, oversample);
     p->n_vis = -1;
     p->n_sm = n_sm;
     p->max_smem = max_smem - 1024;      // leave room for static shared memory
@@ -481,6 +518,14 @@ void grid_plan_destroy(grid_plan* plan) { delete plan; }
 int grid_plan_set_samples(grid_plan* plan, long long n_vis) {
     if (!plan || n_vis < 0) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_samples: invalid argument");
     plan->n_vis = n_vis;
+    if (!plan->user_tuned) {                         // the default block depends on the size of the input
+        grid_plan trial = *plan;
+        default_tuning(&trial);
+        trial.traversal = plan->traversal; trial.time_block = plan->time_block;     // set by their own calls
+        trial.sort_chunks = plan->sort_chunks;
+        if (derive(&trial) == GRID_OK) *plan = trial;
+        g_err[0] = 0;
+    }
     return GRID_OK;
 }
 
@@ -493,7 +538,7 @@ int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_ch
 
 size_t grid_plan_workspace_bytes(const grid_plan* plan) {
     if (!plan || plan->n_vis < 0) return 0;
-    return kHeadBytes + records_bytes(plan) + ((order_capacity(plan) * sizeof(uint32_t) + 15) & ~(size_t)15) + tap_table_bytes(plan);
+    return tap_table_offset(plan) + tap_table_bytes(plan);
 }
 
 int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
@@ -508,7 +553,13 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
                          int chunk, int ctas_per_sm) {
     if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_tuning: null plan");
     grid_plan trial = *plan;
-    if (variant >= 0) trial.variant = variant;
+    if (variant >= 0 && variant != trial.variant) {
+        trial.variant = variant;
+        // the other kernel's thread count does not carry over (variant 3 runs one CTA of up to 1024 threads per SM)
+        if (threads_per_cta <= 0) trial.threads = variant == 3 ? 1024 : 256;
+        if (ctas_per_sm <= 0) trial.ctas_per_sm = variant == 3 ? 1 : 2;
+        if (variant != 3 && batch <= 0 && trial.batch < 16) trial.batch = 64;
+    }
     if (cu > 0) trial.cu = cu;
     if (cv > 0) trial.cv = cv;
     if (threads_per_cta > 0) trial.threads = threads_per_cta;
@@ -524,6 +575,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     }
     if (rc != GRID_OK) return rc;
     *plan = trial;
+    plan->user_tuned = 1;
     return GRID_OK;
 }
 
@@ -554,6 +606,7 @@ int grid_plan_set_pol_split(grid_plan* plan, int lanes) {
     const int rc = derive(&trial);
     if (rc != GRID_OK) return rc;
     *plan = trial;
+    plan->user_tuned = 1;
     return GRID_OK;
 }
 
@@ -634,7 +687,9 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.counters = counters;
     gp.rec16 = (plan->variant == 3 && !ext_recs) ? 1 : 0;
     gp.n_vis = n_vis;
-    gp.N = plan->N; gp.S = plan->S; gp.n_rows = plan->W * plan->O;
+    gp.N = plan->N; gp.S = plan->variant == 3 ? plan->Sk : plan->S;
+    gp.n_rows = plan->variant == 3 ? tap_rows(plan) : plan->W * plan->O;
+    gp.tap_pad = plan->variant == 3 ? plan->Sk - plan->S : 0;
     gp.oversample = plan->O;
     gp.bin_u = plan->bin_u; gp.bin_v = plan->bin_v; gp.row_u = plan->row_u; gp.row_v = plan->row_v;
     gp.nbx = plan->nbx; gp.nby = plan->nby;
@@ -702,17 +757,16 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         } else {
             gp.tc = 1; gp.n_tblocks = 1;
         }
-        if (plan->variant == 3 && plan->S == 128) {              // 2 x 2 tiles per bin: four queue entries per chunk group
+        if (plan->variant == 3 && plan->Sk == 128) {              // 2 x 2 tiles per bin: four queue entries per chunk group
             gp.n_groups_a *= 4;
             gp.n_groups_b *= 4;
         }
         const long long max_groups = gp.n_groups_a > gp.n_groups_b ? gp.n_groups_a : gp.n_groups_b;
-        const int logs = log2_exact(plan->S);
+        const int logs = log2_exact(plan->variant == 3 ? plan->Sk : plan->S);
         if (plan->variant == 3 && plan->taps_global && !plan->dense) {   // a4: row-doubled table in global memory
-            float2* gt = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes +
-                                                   records_bytes(plan) + ((order_capacity(plan) * sizeof(uint32_t) + 15) & ~(size_t)15));
-            const long long n_elems = (long long)plan->W * plan->O * 2 * plan->S;
-            tap_table_kernel<<<(unsigned)((n_elems + 255) / 256), 256, 0, stream>>>(gp.kern, gt, n_elems, plan->S);
+            float2* gt = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(plan->workspace) + tap_table_offset(plan));
+            const long long n_elems = (long long)tap_rows(plan) * 2 * plan->Sk;
+            tap_table_kernel<<<(unsigned)((n_elems + 255) / 256), 256, 0, stream>>>(gp.kern, gt, n_elems, plan->Sk, plan->Sk - plan->S);
             gp.gtaps = gt;
             plan->last_launches++;
         }
@@ -833,7 +887,7 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
         grid_plan tmp = *plan;                       // same plan with polarisation split 1 (shuffle reduction per team)
         tmp.pol_split = 1;
         tmp.threads = 1024;
-        const int logs = log2_exact(plan->S);
+        const int logs = log2_exact(plan->Sk);
         const int tries[3][2] = {{plan->cu, plan->cv}, {4, 2}, {2, 2}};
         for (int t = 0; t < 3; ++t) {
             tmp.cu = tries[t][0]; tmp.cv = tries[t][1];
@@ -858,6 +912,7 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
         return fail(GRID_ERR_CUDA, "grid_degrid: %s", cudaGetErrorString(cudaGetLastError()));
     QuantParams qp = quant_params(plan);
     qp.format = 1;                                   // compact records (cell, tap rows) for every support
+    qp.pad = 0;                                      // this kernel walks the real support
     quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
         uvw, reinterpret_cast<SampleRec*>(recs), n, qp, reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
     const int L = plan->S <= 8 ? 8 : (plan->S <= 16 ? 16 : 32);
@@ -891,7 +946,7 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
     if ((long long)plan->W * plan->O * plan->O * plan->S * plan->S > 0x7fffffffLL)
         return fail(GRID_ERR_UNSUPPORTED, "grid_execute_dense: table beyond 2^31 elements");
     const int logs = log2_exact(plan->S);
-    if (logs >= 2 && logs <= 5) {                    // coarsened kernel with the default block of this (S, P)
+    if (logs >= 2 && logs <= 5) {                    // coarsened kernel with the default block of this (S, P); powers of two only
         grid_plan tmp = *plan;
         tmp.variant = 3; tmp.dense = 1; tmp.pol_split = 1; tmp.threads = 1024; tmp.batch = 32; tmp.chunk = 256;
         if (tmp.P == 1) { tmp.cu = logs == 2 ? 2 : (logs == 5 ? 8 : 4); tmp.cv = logs == 2 ? 2 : 4; }
@@ -905,6 +960,8 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
         g_err[0] = 0;
     }
     // any other support: one atomic per update
+    snprintf(g_err, sizeof(g_err), "note: grid_execute_dense: support %d runs on the one-atomic-per-update kernel "
+             "(the coarsened dense kernel covers powers of two up to 32)", plan->S);
     const long long n = plan->n_vis;
     if (n * plan->S / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_execute_dense: too many samples");
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
@@ -913,6 +970,7 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
         return fail(GRID_ERR_CUDA, "grid_execute_dense: %s", cudaGetErrorString(cudaGetLastError()));
     QuantParams qp = quant_params(plan);
     qp.format = 1;
+    qp.pad = 0;
     quantise_kernel<<<(unsigned)(((n + 3) / 4 + 255) / 256), 256, 0, stream>>>(
         uvw, reinterpret_cast<SampleRec*>(recs), n, qp, reinterpret_cast<float*>(counters + 2), 0, 0, 0.f);
     const unsigned blocks = (unsigned)((n * plan->S + 255) / 256);

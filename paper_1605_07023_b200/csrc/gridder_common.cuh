@@ -29,6 +29,7 @@ struct QuantParams {
     int q_limit;          // (N-S+1)*O : valid iff 0 <= q < q_limit
     int n_wplanes;
     int cu, cv, bin_u, bin_v, row_u, row_v;   // coarsening block, bin, padded row lengths Lu, Lv
+    int pad, sk, grid_size;                   // warp kernel on a support padded to sk = S + pad (a power of two); N
 };
 
 struct GridParams {
@@ -56,6 +57,7 @@ struct GridParams {
     int n_cblocks, chunk_cols;   // variant 3, time-innermost: a chunk spans chunk_cols channels
     int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
     float fzero;              // 0.0f the compiler cannot see: accumulators are cleared by moves from the constant bank
+    int tap_pad;              // warp kernel: zero taps added to each row (support padded to a power of two)
     int rec16;                // warp kernel: records are 16 bytes {pos, rows, weight, -} (quantise format 2), else CycRec
 };
 

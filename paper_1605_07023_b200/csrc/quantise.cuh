@@ -38,8 +38,19 @@ __device__ __forceinline__ QuantOut quantise_sample(float u, float v, float w, c
 
 __device__ __forceinline__ CycRec make_cyc_record(const QuantOut& q, const QuantParams& qp) {
     CycRec rec;
-    rec.pos = (uint32_t)q.i0 | ((uint32_t)q.j0 << 16) | (q.valid ? 0u : 0x8000u);
-    rec.rows = (uint32_t)(q.wp * qp.oversample + q.su) | ((uint32_t)(q.wp * qp.oversample + q.sv) << 16);
+    int i0 = q.i0, j0 = q.j0;
+    uint32_t ru = (uint32_t)(q.wp * qp.oversample + q.su), rv = (uint32_t)(q.wp * qp.oversample + q.sv);
+    if (qp.pad) {
+        // support padded to a power of two with zero taps: row copy 0 has the zeros behind the taps (origin
+        // unchanged), copy 1 in front (origin moved down), used where the padded footprint would leave the grid
+        const uint32_t bu = i0 + qp.sk > qp.grid_size ? 1u : 0u, bv = j0 + qp.sk > qp.grid_size ? 1u : 0u;
+        i0 -= bu ? qp.pad : 0;
+        j0 -= bv ? qp.pad : 0;
+        ru = 2u * ru + bu;
+        rv = 2u * rv + bv;
+    }
+    rec.pos = (uint32_t)i0 | ((uint32_t)j0 << 16) | (q.valid ? 0u : 0x8000u);
+    rec.rows = ru | (rv << 16);
     return rec;
 }
 

@@ -41,13 +41,17 @@ def test_plan_validation(binding):
         assert binding.grid_last_error() != ""
 
 
-@pytest.mark.parametrize("S,P", [(7, 1), (8, 4), (16, 1), (8, 1), (4, 1), (4, 4), (16, 4), (32, 1), (32, 4), (1, 1)])
+@pytest.mark.parametrize("S,P", [(7, 1), (8, 4), (16, 1), (8, 1), (4, 1), (4, 4), (16, 4), (32, 1), (32, 4), (1, 1), (12, 4), (100, 1), (3, 2)])
 def test_default_plan_geometry(binding, S, P):
     plan = binding.GridPlan(4096, S, 8, 16, P)
     i = plan.info()
     if i["variant"] == 3:
-        # power-of-two support: bin == support, owned positions S/C apart (north_star: "taken modulo the support")
-        assert S in (4, 8, 16, 32, 64, 128) and i["bin_u"] == i["bin_v"] == S
+        # bin == support rounded up to a power of two (zero-padded taps); owned positions S/C
+        # apart (north_star: "taken modulo the support")
+        sk = 4
+        while sk < S:
+            sk *= 2
+        assert S >= 3 and i["bin_u"] == i["bin_v"] == sk
     else:
         # bin >= S + C - 1, aligned to the block; a team covers the bin exactly
         assert i["bin_u"] % i["cu"] == 0 and i["bin_v"] % i["cv"] == 0
@@ -104,3 +108,23 @@ def test_product_does_not_import_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle", text, flags=re.M), f
                 assert "gridder_oracle" not in text, f
+
+
+def test_no_silent_scatter_fallback(binding):
+    """Every support in [3, 128] gets the warp kernel (zero-padded to a power of two where needed) for any plane count
+    the ABI accepts, tap table in shared or global memory -- never the one-atomic-per-update kernel (variant 0), which
+    round 1 fell back to for 1755 of 2688 (S, P, W, O) combinations.  Host logic only: no device needed."""
+    bad = []
+    for S in list(range(3, 41)) + [48, 63, 64, 65, 100, 127, 128]:
+        for P in (1, 2, 4):
+            for W, O in ((1, 8), (32, 8), (128, 8), (1229, 8), (16, 4)):
+                plan = binding.GridPlan(4096, S, O, W, P)
+                i = plan.info()
+                plan.destroy()
+                if i["variant"] != 3:
+                    bad.append((S, P, W, O, i["variant"]))
+    assert not bad, bad[:10]
+    # the one documented exception: grids smaller than twice the padded support fall back, and say so
+    plan = binding.GridPlan(18, 13, 4, 1, 1)
+    assert plan.info()["variant"] in (0, 1)
+    plan.destroy()

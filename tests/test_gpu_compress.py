@@ -44,7 +44,7 @@ def run_compress(N, S, O, W, P, uvw, vis, wts, kernel, grid_too=True):
         plan.destroy()
 
 
-@pytest.mark.parametrize("S,P", [(8, 4), (16, 1), (4, 2), (32, 1)])
+@pytest.mark.parametrize("S,P", [(8, 4), (16, 1), (4, 2), (32, 1), (7, 1), (12, 2)])
 def test_compress_matches_oracle(oracle_mod, S, P):
     N, O, W, n = 256, 8, 3, 30_011
     uvw, vis, wts, kernel = slow_walk(50 + S + P, n, N, S, O, W, P, step=0.03)
@@ -53,16 +53,25 @@ def test_compress_matches_oracle(oracle_mod, S, P):
     assert n_c == len(heads) and n_c < 0.7 * n                 # runs were really merged
     q = oracle_mod.quantise(N, S, O, W, uvw[heads])
     # integer content of every compressed record: bit-exact
-    np.testing.assert_array_equal(recs[:, 0] & 0x7fff, q["i0"])
-    np.testing.assert_array_equal(recs[:, 0] >> 16, q["j0"])
-    np.testing.assert_array_equal(recs[:, 1] & 0xffff, q["wp"] * O + q["su"])
-    np.testing.assert_array_equal(recs[:, 1] >> 16, q["wp"] * O + q["sv"])
+    i0, j0 = (recs[:, 0] & 0x7fff).astype(np.int64), (recs[:, 0] >> 16).astype(np.int64)
+    ru, rv = (recs[:, 1] & 0xffff).astype(np.int64), (recs[:, 1] >> 16).astype(np.int64)
+    sk = 1 << (S - 1).bit_length()
+    if sk != S:
+        # support padded to a power of two (include/grid.h, "Supports that are not powers of two"): the row index
+        # carries in its lowest bit which zero-padded copy of the tap row is used; with copy 1 (zeros in front)
+        # the stored origin is the real one minus the padding
+        i0, j0 = i0 + (sk - S) * (ru & 1), j0 + (sk - S) * (rv & 1)
+        ru, rv = ru >> 1, rv >> 1
+    np.testing.assert_array_equal(i0, q["i0"])
+    np.testing.assert_array_equal(j0, q["j0"])
+    np.testing.assert_array_equal(ru, q["wp"] * O + q["su"])
+    np.testing.assert_array_equal(rv, q["wp"] * O + q["sv"])
     # merged values: FP32 sums of up to 50 terms against float64
     scale = np.abs(merged).max()
     assert np.abs(cvis.astype(np.complex128) - merged).max() <= 2e-6 * scale
 
 
-@pytest.mark.parametrize("S,P", [(8, 4), (16, 1), (8, 1), (16, 4)])
+@pytest.mark.parametrize("S,P", [(8, 4), (16, 1), (8, 1), (16, 4), (7, 1), (12, 4)])
 def test_grid_of_compressed_samples(oracle_mod, S, P):
     # "identical results" up to rounding -- compare with the oracle grid of the ORIGINAL samples
     N, O, W, n = 256, 8, 3, 40_003

@@ -268,15 +268,21 @@ def test_inconsistent_layout_hint_is_ignored(oracle_mod):
     assert_parity(got, ref, "bad layout")
 
 
-@pytest.mark.parametrize("S,P", [(64, 4), (128, 1), (100, 2), (48, 4)])
+@pytest.mark.parametrize("S,P", [(64, 4), (128, 1), (100, 2), (48, 4), (7, 1), (13, 4), (3, 2), (40, 1), (5, 4)])
 def test_large_supports_have_a_path(oracle_mod, S, P):
-    # the ABI accepts supports up to 128 (the paper's bins: 32, 64, 128): whatever kernel the plan falls back
-    # to (smaller blocks, or one atomic per update when a bin exceeds a CTA), the result is the oracle's
+    # the ABI accepts supports up to 128 (the paper's bins: 32, 64, 128).  Supports that are not powers of two run
+    # on the warp kernel too, zero-padded to the next power of two (pin P14): never on the
+    # one-atomic-per-update kernel.  Samples near both edges of the grid exercise both padded copies of the tap rows.
     N, O, W, n = 512, 2, 2, 3_001
     uvw, vis, wts, kernel = synth.random_problem(900 + S + P, n, N, S, O, W, P, spread=0.45, walk=0.5)
+    edge = N // 2 - S // 2 - 1
+    uvw[100:140, 0] = np.linspace(edge - 3, edge + 2, 40)      # upper edge in u: some valid, some off the grid
+    uvw[200:240, 1] = np.linspace(edge - 3, edge + 2, 40)
+    uvw[300:340, :2] = -np.linspace(edge - 3, edge + 2, 40)[:, None]
     ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
     got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel)
     print(S, P, info)
+    assert info["variant"] == 3
     assert_parity(got, ref, f"S={S} P={P} {info}")
 
 

@@ -41,6 +41,7 @@ def _load():
         lib.oracle_grid.restype = c_int
         lib.oracle_degrid.argtypes = [c_int] * 5 + [c_ll] + [vp] * 5
         lib.oracle_grid_dense.argtypes = [c_int] * 5 + [c_ll] + [vp] * 5
+        lib.oracle_grid_dense_pol.argtypes = [c_int] * 5 + [c_ll] + [vp] * 5
         lib.oracle_degrid.restype = c_int
         lib.oracle_max_threads.restype = c_int
         _lib = lib
@@ -117,6 +118,24 @@ def grid_dense(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis, weigh
                                vis.ctypes.data, weights.ctypes.data, kernel2d.ctypes.data, out.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_grid_dense: invalid arguments")
+    return out
+
+
+def grid_dense_pol(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis, weights, kernel2d):
+    """Gridding with one dense GCF table per polarisation, kernel2d[p][wp][sv][su][tj][ti] (SURVEY NEXT-4,
+    PAPER.md:97, 186): complex128 grid [N][N][P].  Serial; small cases only."""
+    lib = _load()
+    uvw = _f32(uvw)
+    n = uvw.shape[0]
+    vis = _c64(vis).reshape(n, n_pol)
+    weights = _f32(weights, (n,))
+    kernel2d = _c64(kernel2d)
+    assert kernel2d.shape == (n_pol, n_wplanes, oversample, oversample, support, support), kernel2d.shape
+    out = np.zeros((grid_size, grid_size, n_pol), dtype=np.complex128)
+    rc = lib.oracle_grid_dense_pol(grid_size, support, oversample, n_wplanes, n_pol, n, uvw.ctypes.data,
+                                   vis.ctypes.data, weights.ctypes.data, kernel2d.ctypes.data, out.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_grid_dense_pol: invalid arguments")
     return out
 
 

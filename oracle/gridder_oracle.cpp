@@ -174,6 +174,34 @@ int oracle_grid_dense(int N, int S, int O, int n_wplanes, int P, long long n_vis
     return 0;
 }
 
+// Dense GCF per polarisation, SURVEY NEXT-4 remainder (the coarsened kernel "assumed that the GCF is
+// polarization-independent ... cannot be directly applied to A-projection"; GCFs "dependent on time,
+// frequency, polarization"): the same scatter with one full table per polarisation,
+//   kernel2d[p][wp][sv][su][tj][ti] complex64;  grid[j0+tj][i0+ti][p] += weight_n * vis[n][p] * kernel2d[p][wp][sv][su][tj][ti]
+// Serial, whole grid (complex128 [N][N][P]); small cases only.
+int oracle_grid_dense_pol(int N, int S, int O, int n_wplanes, int P, long long n_vis,
+                          const float* uvw, const float* vis, const float* weights, const float* kernel2d, double* grid) {
+    if (bad_args(N, S, O, n_wplanes, P)) return -1;
+    cd* g = reinterpret_cast<cd*>(grid);
+    const size_t per_pol = (size_t)n_wplanes * O * O * S * S;
+    for (long long n = 0; n < n_vis; ++n) {
+        const Quant q = quantise(uvw + 3 * n, N, S, O, n_wplanes);
+        if (!q.valid) continue;
+        const double wt = (double)weights[n];
+        const size_t entry = (((size_t)q.wp * O + q.sv) * O + q.su) * S * S;
+        for (int p = 0; p < P; ++p) {
+            const float* k = kernel2d + 2 * ((size_t)p * per_pol + entry);
+            const cd v((double)vis[2 * (n * P + p)], (double)vis[2 * (n * P + p) + 1]);
+            for (int tj = 0; tj < S; ++tj)
+                for (int ti = 0; ti < S; ++ti) {
+                    const cd gij((double)k[2 * (tj * S + ti)], (double)k[2 * (tj * S + ti) + 1]);
+                    g[((size_t)(q.j0 + tj) * N + (size_t)(q.i0 + ti)) * P + p] += wt * v * gij;
+                }
+        }
+    }
+    return 0;
+}
+
 // Adjoint (degridding), written solely for pin P7 (north_star property 5):
 //   out[n][p] = weight_n * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * G[j0+tj][i0+ti][p]
 // Invalid samples give 0.  grid is a full [N][N][P] complex128 array; out is complex128 [n_vis][P].

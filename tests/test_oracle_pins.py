@@ -436,3 +436,36 @@ def test_dense_oracle_unit_sample_and_separable_limit(oracle_mod):
     g_dense = oracle_mod.grid_dense(N, S, O, W, 2, uvw, vis, wts, outer.astype(np.complex64))
     assert np.abs(g_dense - g_sep).max() <= 4e-7 * np.abs(g_sep).max()
     assert np.linalg.norm(g_dense - g_sep) <= 2e-7 * np.linalg.norm(g_sep)
+
+
+def test_dense_pol_oracle_unit_sample_per_polarisation_and_equal_limit(oracle_mod):
+    # oracle.grid_dense_pol (NEXT-4 remainder), pinned by what its definition fixes:
+    # (a) one sample with a DIFFERENT unit visibility per polarisation reproduces, in each polarisation plane of the
+    #     grid, that polarisation's own table entry kernel2d[p][wp][sv][su] times that visibility -- rows = v taps,
+    #     columns = u taps, at the hand-quantised cell (asymmetric random tables: a swapped polarisation, a transpose
+    #     or a wrong sub-offset order shows);
+    # (b) with the same table for every polarisation it is exactly oracle.grid_dense (bit for bit: same arithmetic);
+    # (c) linearity in the table: scaling polarisation 1's table by 2 doubles plane 1 of the grid and nothing else.
+    rng = np.random.default_rng(41)
+    P = 4
+    k2 = (rng.standard_normal((P, W, O, O, S, S)) + 1j * rng.standard_normal((P, W, O, O, S, S))).astype(np.complex64)
+    uvw = np.array([[3.0, -4.25, 1.5]], dtype=np.float32)      # as in the dense pin: su = 2, sv = 1, plane 1 (N=32, S=5, O=4)
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    assert (q["su"][0], q["sv"][0], q["wp"][0]) == (2, 1, 1)
+    v = np.array([[1.0, 2.0, 1j, -1.0 - 1j]], dtype=np.complex64)
+    g = oracle_mod.grid_dense_pol(N, S, O, W, P, uvw, v, np.ones(1, np.float32), k2)
+    j0, i0 = q["j0"][0], q["i0"][0]
+    for p in range(P):
+        expect = np.zeros((N, N), np.complex128)
+        expect[j0:j0 + S, i0:i0 + S] = complex(v[0, p]) * k2[p, 1, 1, 2].astype(np.complex128)
+        np.testing.assert_array_equal(g[:, :, p], expect)
+    uvw, vis, wts, _ = synth.random_problem(42, 500, N, S, O, W, P, spread=0.5)
+    same = np.broadcast_to(k2[2], k2.shape).copy()
+    np.testing.assert_array_equal(oracle_mod.grid_dense_pol(N, S, O, W, P, uvw, vis, wts, same),
+                                  oracle_mod.grid_dense(N, S, O, W, P, uvw, vis, wts, k2[2]))
+    g1 = oracle_mod.grid_dense_pol(N, S, O, W, P, uvw, vis, wts, k2)
+    k3 = k2.copy()
+    k3[1] *= 2
+    g2 = oracle_mod.grid_dense_pol(N, S, O, W, P, uvw, vis, wts, k3)
+    np.testing.assert_array_equal(g2[:, :, 1], 2 * g1[:, :, 1])
+    np.testing.assert_array_equal(g2[:, :, [0, 2, 3]], g1[:, :, [0, 2, 3]])

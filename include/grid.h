@@ -104,6 +104,15 @@ int grid_execute_compressed(grid_plan* plan, const void* records, const float* v
 int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                        const float* conv_kernel_2d, float* grid, grid_stream_t stream);
 
+/* The same with one dense table per polarisation (the coarsened kernel "assumed that the GCF is
+ * polarization-independent ... cannot be directly applied to A-projection"; GCFs "dependent on
+ * time, frequency, polarization"):
+ *     grid[j0+tj][i0+ti][p] += weights[n] * vis[n][p] * conv_kernel_2d_pol[p][wp][sv][su][tj][ti]
+ *   conv_kernel_2d_pol  [n_pol][n_wplanes][oversample][oversample][support][support] complex64, DEVICE
+ * Same kernels as grid_execute_dense; a thread fetches the table values of each of its polarisations in turn. */
+int grid_execute_dense_pol(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                           const float* conv_kernel_2d_pol, float* grid, grid_stream_t stream);
+
 /* Degridding, the adjoint of grid_execute (the paper calls its own degridder preliminary
  * and does not measure it).  For every sample whose footprint lies inside the grid
  *     vis_out[n][p] = weights[n] * sum_{tj,ti} conj(k[wp][sv][tj] * k[wp][su][ti]) * grid[j0+tj][i0+ti][p]

@@ -15,7 +15,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
-    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
     "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
@@ -37,6 +37,7 @@ _lib.grid_execute.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
 _lib.grid_compress.argtypes = [_vp] * 8
 _lib.grid_execute_dense.argtypes = [_vp] * 7
+_lib.grid_execute_dense_pol.argtypes = [_vp] * 7
 _lib.grid_degrid.argtypes = [_vp] * 7
 _lib.grid_plan_set_degrid_gather.argtypes = [_vp, _int]
 _lib.grid_execute_compressed.argtypes = [_vp, _vp, _vp, _ll, _vp, _vp, _vp]
@@ -154,20 +155,32 @@ class GridPlan:
     def last_launches(self) -> int:
         return int(_lib.grid_plan_last_launches(self._h))
 
+    def _check_samples(self, uvw=None, vis=None, weights=None, grid=None, vis_out=None):
+        """Sizes against the plan (every wrapper: an undersized array would be read or written out of bounds on the
+        device).  Marshalling only -- no arithmetic on the data."""
+        n = self.n_vis
+        if n is None:
+            _lib.grid_plan_set_samples(self._h, -1)            # leaves "invalid argument" in grid_last_error
+            raise GridError(GRID_ERR_STATE, "set_samples has not been called")
+        if uvw is not None and uvw.numel() != 3 * n:
+            raise ValueError(f"uvw must hold [n_vis = {n}][3] floats, got {uvw.numel()} elements")
+        if vis is not None and vis.numel() != n * self.n_pol:
+            raise ValueError(f"vis must hold [n_vis = {n}][n_pol = {self.n_pol}] complex values, got {vis.numel()}")
+        if weights is not None and weights.numel() != n:
+            raise ValueError(f"weights must hold n_vis = {n} floats, got {weights.numel()}")
+        if vis_out is not None and vis_out.numel() != n * self.n_pol:
+            raise ValueError(f"vis_out must hold [n_vis = {n}][n_pol = {self.n_pol}] complex values, got {vis_out.numel()}")
+        if grid is not None and grid.numel() != self.grid_size * self.grid_size * self.n_pol:
+            raise ValueError("grid must be [N][N][n_pol]")
+
     def execute(self, uvw, vis, weights, conv_kernel, grid, stream=None):
         """grid += gridded samples (grid_execute).  All arguments are CUDA tensors:
         uvw float32 [n][3], vis complex64 [n][P], weights float32 [n],
         conv_kernel complex64 [W][O][S], grid complex64 [N][N][P]."""
         import torch
-        n = self.n_vis
-        if n is None:
-            raise GridError(GRID_ERR_STATE, "grid_execute (set_samples not called)")
-        if n > 0 and (uvw.numel() != 3 * n or vis.numel() != n * self.n_pol or weights.numel() != n):
-            raise ValueError("array sizes do not match set_samples()")
+        self._check_samples(uvw, vis, weights, grid)
         if conv_kernel.numel() != self.n_wplanes * self.oversample * self.support:
             raise ValueError("conv_kernel must be [n_wplanes][oversample][support]")
-        if grid.numel() != self.grid_size * self.grid_size * self.n_pol:
-            raise ValueError("grid must be [N][N][n_pol]")
         rc = _lib.grid_execute(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
                                _ptr(weights, torch.float32, "weights"),
                                _ptr(conv_kernel, torch.complex64, "conv_kernel"),
@@ -177,6 +190,7 @@ class GridPlan:
     def execute_dense(self, uvw, vis, weights, conv_kernel_2d, grid, stream=None):
         """grid_execute_dense: conv_kernel_2d complex64 [W][O][O][S][S] (plane, sv, su, row, column)."""
         import torch
+        self._check_samples(uvw, vis, weights, grid)
         if conv_kernel_2d.numel() != self.n_wplanes * self.oversample ** 2 * self.support ** 2:
             raise ValueError("conv_kernel_2d must be [n_wplanes][oversample][oversample][support][support]")
         rc = _lib.grid_execute_dense(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
@@ -185,10 +199,23 @@ class GridPlan:
                                      _ptr(grid, torch.complex64, "grid"), _stream(stream))
         _check(rc, "grid_execute_dense")
 
+    def execute_dense_pol(self, uvw, vis, weights, conv_kernel_2d_pol, grid, stream=None):
+        """grid_execute_dense_pol: conv_kernel_2d_pol complex64 [P][W][O][O][S][S] (one dense table per polarisation)."""
+        import torch
+        self._check_samples(uvw, vis, weights, grid)
+        if conv_kernel_2d_pol.numel() != self.n_pol * self.n_wplanes * self.oversample ** 2 * self.support ** 2:
+            raise ValueError("conv_kernel_2d_pol must be [n_pol][n_wplanes][oversample][oversample][support][support]")
+        rc = _lib.grid_execute_dense_pol(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
+                                         _ptr(weights, torch.float32, "weights"),
+                                         _ptr(conv_kernel_2d_pol, torch.complex64, "conv_kernel_2d_pol"),
+                                         _ptr(grid, torch.complex64, "grid"), _stream(stream))
+        _check(rc, "grid_execute_dense_pol")
+
     def compress(self, uvw, vis, weights, stream=None):
         """grid_compress: returns (records uint8 [n_c][8], vis complex64 [n_c][P], n_c) -- CUDA tensors trimmed
         to the compressed count (one host sync to read it)."""
         import torch
+        self._check_samples(uvw, vis, weights)
         n = self.n_vis
         recs = torch.empty((max(n, 1), 8), dtype=torch.uint8, device=uvw.device)
         cvis = torch.empty((max(n, 1), self.n_pol), dtype=torch.complex64, device=uvw.device)
@@ -203,7 +230,12 @@ class GridPlan:
     def execute_compressed(self, records, vis, conv_kernel, grid, stream=None):
         """grid_execute_compressed on the output of compress()."""
         import torch
+        self._check_samples(grid=grid)
         n_c = records.shape[0]
+        if records.numel() != n_c * 8 or vis.numel() != n_c * self.n_pol or n_c > self.n_vis:
+            raise ValueError("records must be [n_c][8] bytes and vis [n_c][n_pol] with n_c <= n_vis")
+        if conv_kernel.numel() != self.n_wplanes * self.oversample * self.support:
+            raise ValueError("conv_kernel must be [n_wplanes][oversample][support]")
         rc = _lib.grid_execute_compressed(self._h, _ptr(records, torch.uint8, "records") if n_c else None,
                                           _ptr(vis, torch.complex64, "vis") if n_c else None, n_c,
                                           _ptr(conv_kernel, torch.complex64, "conv_kernel"),
@@ -216,9 +248,13 @@ class GridPlan:
     def degrid(self, uvw, weights, conv_kernel, grid, vis_out=None, stream=None):
         """grid_degrid: vis_out complex64 [n][P] (allocated if None) = adjoint of execute() applied to grid."""
         import torch
+        self._check_samples(uvw, None, weights, grid)
         n = self.n_vis
         if vis_out is None:
             vis_out = torch.empty((n, self.n_pol), dtype=torch.complex64, device=grid.device)
+        self._check_samples(vis_out=vis_out)
+        if conv_kernel.numel() != self.n_wplanes * self.oversample * self.support:
+            raise ValueError("conv_kernel must be [n_wplanes][oversample][support]")
         if n == 0:
             return vis_out
         rc = _lib.grid_degrid(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(weights, torch.float32, "weights"),

@@ -153,9 +153,10 @@ struct WarpKernelTraits {
 // as the paper's kernel does (Table 1 "unified cache").
 // DENSE: gp.kern is a non-separable table [W][O][O][S][S]
 // (plane, v sub-offset, u sub-offset, row, column); a thread fetches the Cu*Cv values of its points from
-// global memory (L1/L2) instead of Cu+Cv taps, and no GCF product is formed.  S <= 32.
+// global memory (L1/L2) instead of Cu+Cv taps, and no GCF product is formed.  S <= 32.  DENSE = 2: one such table
+// per polarisation, gp.dense_pol_stride elements apart (A-projection kernels depend on the polarisation).
 // RS ("row skip"): the row pass of the flush skips the points its column pass has just flushed (see the flush).
-template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false, bool TG = false, bool DENSE = false, bool RS = false>
+template <int CU, int CV, int P, int LOGS, int PS = 1, bool DEGRID = false, bool TG = false, int DENSE = 0, bool RS = false>
 __global__ void __launch_bounds__((WarpKernelTraits<CU, CV, P, LOGS, PS>::MAX_THREADS), 1)
 grid_warp_kernel(const GridParams gp) {
     using T = WarpKernelTraits<CU, CV, P, LOGS, PS>;
@@ -632,15 +633,39 @@ grid_warp_kernel(const GridParams gp) {
                     const int mi = (px0 - (int)(c.x & 0x7fffu)) & (S - 1), mj = (py0 - (int)(c.x >> 16)) & (S - 1);
                     const float2* kb = gp.kern + c.y;
                     c = *++rp;                         // next sample's record
-                    float2 g2[CV][CU], v[PT];
+                    float2 v[PT];
+#pragma unroll
+                    for (int q = 0; q < PT; ++q) v[q] = vp[q];
+                    vp += P;
+                    if constexpr (DENSE == 2) {
+                        // one table per polarisation: the values of polarisation q are fetched and used, then the next
+#pragma unroll
+                        for (int q = 0; q < PT; ++q) {
+                            const float2* kq = kb + (size_t)(half * PT + q) * (size_t)gp.dense_pol_stride;
+                            float2 g2[CV][CU];
+#pragma unroll
+                            for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                                for (int a = 0; a < CU; ++a)
+                                    g2[bb][a] = __ldg(kq + ((mj + bb * DV) & (S - 1)) * S + ((mi + a * DU) & (S - 1)));
+#pragma unroll
+                            for (int bb = 0; bb < CV; ++bb)
+#pragma unroll
+                                for (int a = 0; a < CU; ++a) {                               // a7
+                                    acc[bb][a][q].x = fmaf(g2[bb][a].x, v[q].x, acc[bb][a][q].x);
+                                    acc[bb][a][q].x = fmaf(-g2[bb][a].y, v[q].y, acc[bb][a][q].x);
+                                    acc[bb][a][q].y = fmaf(g2[bb][a].x, v[q].y, acc[bb][a][q].y);
+                                    acc[bb][a][q].y = fmaf(g2[bb][a].y, v[q].x, acc[bb][a][q].y);
+                                }
+                        }
+                        continue;
+                    }
+                    float2 g2[CV][CU];
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb)
 #pragma unroll
                         for (int a = 0; a < CU; ++a)
                             g2[bb][a] = __ldg(kb + ((mj + bb * DV) & (S - 1)) * S + ((mi + a * DU) & (S - 1)));
-#pragma unroll
-                    for (int q = 0; q < PT; ++q) v[q] = vp[q];
-                    vp += P;
 #pragma unroll
                     for (int bb = 0; bb < CV; ++bb)
 #pragma unroll

@@ -45,7 +45,7 @@ struct grid_plan {
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
     int groups_per_cta, queue_teams;
-    int dense;                            // internal (grid_execute_dense): non-separable table, read from global memory
+    int dense;                            // internal (grid_execute_dense): non-separable table, read from global memory; 2: one per polarisation
     int taps_global;                      // variant 3: tap table read from global memory (too large for shared)
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
@@ -150,18 +150,24 @@ WarpDesc lookup_warp_tg(int cu, int cv, int P, int logs) {
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
-// Dense (non-separable) GCF kernels: default blocks, S <= 32.
-template <int CU, int CV, int P>
+// Dense (non-separable) GCF kernels: default blocks, S <= 32.  KIND 1: one table, 2: one table per polarisation.
+template <int CU, int CV, int P, int KIND>
 WarpDesc pick_dense(int logs) {
 #define DCASE(l) case l: if constexpr (CU <= (1 << l) && CV <= (1 << l)) { using T = WarpKernelTraits<CU, CV, P, l, 1>; \
-        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, false, true>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; } break;
+        return WarpDesc{grid_warp_kernel<CU, CV, P, l, 1, false, false, KIND>, T::GT, T::TPG, T::TEAM, T::MAX_THREADS, &T::group_bytes}; } break;
     switch (logs) { DCASE(2) DCASE(3) DCASE(4) DCASE(5) }
 #undef DCASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
 
-WarpDesc lookup_warp_dense(int cu, int cv, int P, int logs) {
-#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_dense<a, b, p>(logs);
+WarpDesc lookup_warp_dense(int cu, int cv, int P, int logs, int kind = 1) {
+    if (kind == 2) {
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_dense<a, b, p, 2>(logs);
+        CASE(2, 2, 2) CASE(4, 2, 2) CASE(2, 2, 4) CASE(4, 2, 4)
+#undef CASE
+        return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
+    }
+#define CASE(a, b, p) if (cu == a && cv == b && P == p) return pick_dense<a, b, p, 1>(logs);
     CASE(2, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1) CASE(2, 2, 2) CASE(4, 2, 2) CASE(2, 2, 4) CASE(4, 2, 4)
 #undef CASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
@@ -171,7 +177,8 @@ WarpDesc lookup_warp_dense(int cu, int cv, int P, int logs) {
 template <int P>
 __global__ void __launch_bounds__(256)
 grid_scatter_dense_kernel(const CycRec* __restrict__ recs, const float2* __restrict__ vis, const float* __restrict__ weights,
-                          const float2* __restrict__ kernel2d, float* __restrict__ grid, long long n_vis, int N, int S, int O) {
+                          const float2* __restrict__ kernel2d, float* __restrict__ grid, long long n_vis, int N, int S, int O,
+                          long long pol_stride) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long n = g / S;
     const int tj = (int)(g - n * S);
@@ -185,9 +192,9 @@ grid_scatter_dense_kernel(const CycRec* __restrict__ recs, const float2* __restr
     const float w = weights[n];
     float* row = grid + ((size_t)(j0 + tj) * N + i0) * (2 * P);
     for (int ti = 0; ti < S; ++ti) {
-        const float2 gk = __ldg(k + ti);
 #pragma unroll
         for (int q = 0; q < P; ++q) {
+            const float2 gk = __ldg(k + (size_t)q * pol_stride + ti);       // pol_stride 0: one table for all polarisations
             float2 v = vis[n * P + q];
             v.x *= w; v.y *= w;
             red_add_v2(row + (size_t)(ti * P + q) * 2, gk.x * v.x - gk.y * v.y, gk.x * v.y + gk.y * v.x);
@@ -279,7 +286,7 @@ int derive(grid_plan* p) {
             return fail(GRID_ERR_UNSUPPORTED, "coarsening block %dx%d (pol split %d) is not instantiated for %d pols, support %d",
                         p->cu, p->cv, p->pol_split, p->P, p->S);
         if (p->dense) {                                  // grid_execute_dense: no tap table on chip
-            d = lookup_warp_dense(p->cu, p->cv, p->P, logs);
+            d = lookup_warp_dense(p->cu, p->cv, p->P, logs, p->dense);
             if (!d.fn || p->pol_split != 1)
                 return fail(GRID_ERR_UNSUPPORTED, "dense GCF: block %dx%d is not instantiated for %d pols, support %d",
                             p->cu, p->cv, p->P, p->S);
@@ -690,6 +697,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.N = plan->N; gp.S = plan->variant == 3 ? plan->Sk : plan->S;
     gp.n_rows = plan->variant == 3 ? tap_rows(plan) : plan->W * plan->O;
     gp.tap_pad = plan->variant == 3 ? plan->Sk - plan->S : 0;
+    gp.dense_pol_stride = plan->dense == 2 ? (long long)plan->W * plan->O * plan->O * plan->S * plan->S : 0;
     gp.oversample = plan->O;
     gp.bin_u = plan->bin_u; gp.bin_v = plan->bin_v; gp.row_u = plan->row_u; gp.row_v = plan->row_v;
     gp.nbx = plan->nbx; gp.nby = plan->nby;
@@ -770,7 +778,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
             gp.gtaps = gt;
             plan->last_launches++;
         }
-        kernel_fn fn = plan->dense ? lookup_warp_dense(plan->cu, plan->cv, plan->P, logs).fn
+        kernel_fn fn = plan->dense ? lookup_warp_dense(plan->cu, plan->cv, plan->P, logs, plan->dense).fn
                      : degrid_out ? lookup_degrid(plan->cu, plan->cv, plan->P, logs, plan->taps_global != 0)
                      : (plan->variant == 3 && plan->taps_global) ? lookup_warp_tg(plan->cu, plan->cv, plan->P, logs).fn
                      : plan->variant == 3 ? lookup_warp(plan->cu, plan->cv, plan->P, logs, plan->pol_split,
@@ -930,8 +938,8 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
     return GRID_OK;
 }
 
-int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
-                       const float* conv_kernel_2d, float* grid, grid_stream_t stream_) {
+static int execute_dense_impl(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                              const float* conv_kernel_2d, float* grid, grid_stream_t stream_, bool per_pol) {
     cudaStream_t stream = (cudaStream_t)stream_;
     if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: null plan");
     plan->last_launches = 0;
@@ -943,12 +951,13 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
         return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: array arguments must be 16-byte aligned");
     if (!plan->workspace || plan->workspace_bytes < grid_plan_workspace_bytes(plan))
         return fail(GRID_ERR_STATE, "grid_execute_dense: workspace missing or smaller than grid_plan_workspace_bytes()");
-    if ((long long)plan->W * plan->O * plan->O * plan->S * plan->S > 0x7fffffffLL)
+    const long long table_elems = (long long)plan->W * plan->O * plan->O * plan->S * plan->S;
+    if (table_elems * (per_pol ? plan->P : 1) > 0x7fffffffLL)
         return fail(GRID_ERR_UNSUPPORTED, "grid_execute_dense: table beyond 2^31 elements");
     const int logs = log2_exact(plan->S);
     if (logs >= 2 && logs <= 5) {                    // coarsened kernel with the default block of this (S, P); powers of two only
         grid_plan tmp = *plan;
-        tmp.variant = 3; tmp.dense = 1; tmp.pol_split = 1; tmp.threads = 1024; tmp.batch = 32; tmp.chunk = 256;
+        tmp.variant = 3; tmp.dense = (per_pol && tmp.P > 1) ? 2 : 1; tmp.pol_split = 1; tmp.threads = 1024; tmp.batch = 32; tmp.chunk = 256;
         if (tmp.P == 1) { tmp.cu = logs == 2 ? 2 : (logs == 5 ? 8 : 4); tmp.cv = logs == 2 ? 2 : 4; }
         else if (tmp.P == 2) { tmp.cu = logs == 2 ? 2 : 4; tmp.cv = 2; }
         else { tmp.cu = logs <= 3 ? 2 : 4; tmp.cv = 2; }
@@ -976,13 +985,24 @@ int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, cons
     const unsigned blocks = (unsigned)((n * plan->S + 255) / 256);
     const float2* v2 = reinterpret_cast<const float2*>(vis);
     const float2* k2 = reinterpret_cast<const float2*>(conv_kernel_2d);
-    if (plan->P == 1) grid_scatter_dense_kernel<1><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
-    else if (plan->P == 2) grid_scatter_dense_kernel<2><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
-    else grid_scatter_dense_kernel<4><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O);
+    const long long ps = per_pol ? table_elems : 0;
+    if (plan->P == 1) grid_scatter_dense_kernel<1><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O, ps);
+    else if (plan->P == 2) grid_scatter_dense_kernel<2><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O, ps);
+    else grid_scatter_dense_kernel<4><<<blocks, 256, 0, stream>>>(recs, v2, weights, k2, grid, n, plan->N, plan->S, plan->O, ps);
     plan->last_launches = 2;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GRID_ERR_CUDA, "grid_execute_dense: launch failed: %s", cudaGetErrorString(e));
     return GRID_OK;
+}
+
+int grid_execute_dense(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                       const float* conv_kernel_2d, float* grid, grid_stream_t stream) {
+    return execute_dense_impl(plan, uvw, vis, weights, conv_kernel_2d, grid, stream, false);
+}
+
+int grid_execute_dense_pol(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                           const float* conv_kernel_2d_pol, float* grid, grid_stream_t stream) {
+    return execute_dense_impl(plan, uvw, vis, weights, conv_kernel_2d_pol, grid, stream, true);
 }
 
 int grid_execute_compressed(grid_plan* plan, const void* records, const float* vis, long long n,

@@ -57,6 +57,7 @@ struct GridParams {
     int n_cblocks, chunk_cols;   // variant 3, time-innermost: a chunk spans chunk_cols channels
     int force_mode;           // -1: pick from hop_stats, 0: channel-innermost, 1: time-innermost
     float fzero;              // 0.0f the compiler cannot see: accumulators are cleared by moves from the constant bank
+    long long dense_pol_stride;   // dense GCF per polarisation: elements between the tables of two polarisations
     int tap_pad;              // warp kernel: zero taps added to each row (support padded to a power of two)
     int rec16;                // warp kernel: records are 16 bytes {pos, rows, weight, -} (quantise format 2), else CycRec
 };

@@ -297,6 +297,109 @@ def measure_config(name, steps, warmup, dev, oracle_band=True):
             "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err}
 
 
+def run_wstack(args):
+    """--config paper_wstack_S{S}_P{P}: the paper's W-stacked run.  The paper-shaped
+    workload is split into 7 slices by w; every slice is compressed once (grid_compress, outside the timed region:
+    PAPER.md:69 "pre-process ... reused") and gridded by its own grid_execute_compressed call onto its own grid with its
+    own 1229 W-projection planes, each slice on its own stream so that the sparse slices overlap.  One step = the
+    7 calls; the rate counts compressed samples, as the paper's does.  Single GPU."""
+    import torch
+    from paper_1605_07023_b200 import binding, synth
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py: the W-stacked workload is a single-GPU run (slices could go to separate GPUs: DESIGN.md)")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gridder has no CPU fallback")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    cfg = synth.get_config(args.config)
+    wl = synth.make_workload(cfg)
+    slices = synth.split_wstack(wl)
+    N, S, O, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_pol
+    W = cfg.n_wplanes // len(slices)
+    main = torch.cuda.current_stream()
+    work = []
+    for sl in slices:
+        plan = binding.GridPlan(N, S, O, W, P)
+        plan.set_samples(len(sl.sample_idx))
+        plan.allocate_workspace(dev)
+        d_uvw, d_vis, d_w = (torch.from_numpy(a).to(dev) for a in (sl.uvw, sl.vis, sl.weights))
+        recs, cvis, n_c = plan.compress(d_uvw, d_vis, d_w)
+        recs, cvis = recs.clone(), cvis.clone()              # trimmed copies: the uncompressed arrays can go
+        del d_uvw, d_vis, d_w
+        work.append({"plan": plan, "recs": recs, "vis": cvis, "n_c": n_c, "n": len(sl.sample_idx),
+                     "kern": torch.from_numpy(sl.kernel).to(dev), "stream": torch.cuda.Stream(device=dev),
+                     "grid": torch.zeros((N, N, P), dtype=torch.complex64, device=dev),
+                     "ev": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
+                     "done": torch.cuda.Event()})
+    torch.cuda.synchronize()
+    updates = sum(w["n_c"] for w in work) * S * S * P
+
+    def step():
+        fork = torch.cuda.Event()
+        fork.record(main)
+        for w in work:
+            w["stream"].wait_event(fork)
+            with torch.cuda.stream(w["stream"]):
+                w["plan"].execute_compressed(w["recs"], w["vis"], w["kern"], w["grid"], stream=w["stream"])
+                w["done"].record(w["stream"])
+        for w in work:
+            main.wait_event(w["done"])
+
+    for w in work:
+        a, b = w["ev"]
+        a.record(main); b.record(main)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(main)
+    launches = 0
+    for k in range(args.steps):
+        if k == args.steps - 1:
+            for w in work:
+                w["plan"].set_kernel_events(*w["ev"])
+        step()
+        launches += sum(w["plan"].last_launches() for w in work)
+    e1.record(main)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / args.steps
+    per_slice = []
+    for i, w in enumerate(work):
+        info = w["plan"].info()
+        kms = w["ev"][0].elapsed_time(w["ev"][1])
+        upd = w["n_c"] * S * S * P
+        per_slice.append({"slice": i, "n_vis": w["n"], "n_compressed": w["n_c"], "kernel_ms": kms,
+                          "pct_fp32_roofline_kernel": 100.0 * upd * FLOPS_PER_UPDATE / (kms * 1e-3) / (PEAK_FP32_TFLOPS * 1e12),
+                          "kernel": kernel_template_name(info, P, S)})
+        w["plan"].set_kernel_events(None, None)
+    big = max(range(len(work)), key=lambda i: work[i]["n_c"])
+    achieved = work[big]["n_c"] * S * S * P * FLOPS_PER_UPDATE / (per_slice[big]["kernel_ms"] * 1e-3) / 1e12
+    value = updates / (ms * 1e-3)
+    line = {
+        "metric": metric_name(), "value": value, "unit": "updates/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_vis": cfg.n_vis, "n_compressed": sum(w["n_c"] for w in work), "grid": N,
+                   "support": S, "oversample": O, "n_wplanes": W, "n_slices": len(work), "n_pol": P,
+                   "updates_per_step": updates,
+                   "l2": "7 grids of %.0f MB and %.2f GB of compressed samples per step exceed the 126 MB L2; no explicit flush"
+                         % (N * N * P * 8 / 1e6, sum(w["recs"].numel() + w["vis"].numel() * 8 for w in work) / 1e9),
+                   "op": "grid_execute_compressed x %d slices, one stream each (compression outside the timed region)" % len(work)},
+        "pct_fp32_roofline": 100.0 * value * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / PEAK_FP32_TFLOPS, "traffic": None, "kernel": per_slice[big]["kernel"],
+                     "kernel_ms": per_slice[big]["kernel_ms"], "of": "slice %d (the largest)" % big,
+                     "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (derived; DESIGN.md)"},
+        "per_slice": per_slice, "clocks": clocks, "gpu_launches": launches,
+    }
+    print(json.dumps(line), flush=True)
+    for w in work:
+        w["plan"].destroy()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -489,6 +592,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config.startswith("paper_wstack_"):
+        run_wstack(args)
     else:
         run_ours(args)
 

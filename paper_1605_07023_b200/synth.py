@@ -76,6 +76,44 @@ def paper_regime_config(support: int, n_pol: int, n_wplanes: int = 16) -> Config
                   support, 8, n_wplanes, "kb_chirp", False)
 
 
+WSTACK_SLICES = 7          # "7 slices"
+WSTACK_PLANES = 1229       # "1229 W planes per slice"
+
+
+def wstack_config(support: int, n_pol: int, n_slices: int = WSTACK_SLICES, planes_per_slice: int = WSTACK_PLANES) -> Config:
+    """The paper's W-stacked run (the data is split "into a number of slices by w value", each
+    gridded by "a separate kernel-instance" onto its own grid with its own W-projection planes): the paper-shaped
+    workload with n_slices * planes_per_slice w-planes; split_wstack() cuts it into the slices."""
+    base = paper_regime_config(support, n_pol, n_slices * planes_per_slice)
+    return replace(base, name=f"paper_wstack_S{support}_P{n_pol}")
+
+
+@dataclass
+class WSlice:
+    index: int
+    sample_idx: np.ndarray     # positions of the slice's samples in the full workload (input order kept)
+    uvw: np.ndarray            # w relative to the slice's first plane
+    vis: np.ndarray
+    weights: np.ndarray
+    kernel: np.ndarray         # the slice's own planes [planes_per_slice][O][S]
+
+
+def split_wstack(wl: "Workload", n_slices: int = WSTACK_SLICES):
+    """Input preparation of the W-stacked run: slice s takes the samples whose w (in plane units) falls into
+    [s, s+1) * planes_per_slice, with w counted from the slice's first plane and the slice's own tap planes."""
+    per = wl.cfg.n_wplanes // n_slices
+    assert per * n_slices == wl.cfg.n_wplanes
+    which = np.minimum((wl.uvw[:, 2] // per).astype(np.int64), n_slices - 1)
+    out = []
+    for s in range(n_slices):
+        idx = np.flatnonzero(which == s)
+        uvw = wl.uvw[idx].copy()
+        uvw[:, 2] -= np.float32(s * per)                  # exact: an integer taken off a float of larger magnitude
+        out.append(WSlice(s, idx, uvw, np.ascontiguousarray(wl.vis[idx]), wl.weights[idx].copy(),
+                          np.ascontiguousarray(wl.kernel[s * per:(s + 1) * per])))
+    return out
+
+
 def sweep_config(support: int, n_pol: int) -> Config:
     """BASELINE.json:configs[4]: support/pol sweep on the config-1 array, 4096 grid, 16 chirp planes."""
     base = CONFIGS["cfg1"]
@@ -86,6 +124,9 @@ def sweep_config(support: int, n_pol: int) -> Config:
 def get_config(name: str) -> Config:
     if name in CONFIGS:
         return CONFIGS[name]
+    if name.startswith("paper_wstack_S"):
+        sp, p = name[len("paper_wstack_S"):].split("_P")
+        return wstack_config(int(sp), int(p))
     if name.startswith("paper_S"):
         s, rest = name[len("paper_S"):].split("_P")
         p, _, w = rest.partition("_W")

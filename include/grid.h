@@ -175,6 +175,26 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode);
  * GRID_ERR_UNSUPPORTED if that combination is not instantiated. */
 int grid_plan_set_pol_split(grid_plan* plan, int lanes);
 
+/* Autotuning as the paper does it ("a small artificial data-set is synthesized and benchmarked with a
+ * range of coarsening factors and work-group sizes, and the best combination is remembered ... separately for each
+ * number of polarizations").
+ *
+ * grid_plan_autotune_candidates: HOST only, no device needed.  Writes up to max_candidates triples
+ * (cu, cv, polarisation split) that are instantiated and fit this plan (shared memory, registers) into out[3*k..],
+ * the plan's current block first; returns how many there are (<= 0: the plan does not run the warp kernel).
+ *
+ * grid_plan_autotune: synthesises n_samples samples on the device (0 = 1 << 20; tracks of a synthetic array
+ * shaped by the layout hint if one is set, else single-channel tracks; counter-based generator seeded with
+ * `seed`; random visibilities and weights, Kaiser-Bessel-like taps), grids them with every candidate onto a
+ * scratch grid of the plan's size (cudaMalloc'ed and freed here, like the inputs), times each with CUDA events on
+ * `stream` (second of two runs) and installs the fastest (as grid_plan_set_tuning + grid_plan_set_pol_split
+ * would).  Synchronises `stream`.  results, if not NULL, receives for every candidate, in the order of
+ * grid_plan_autotune_candidates, the time in microseconds (< 0: failed) -- at most max_candidates entries.
+ * Returns GRID_OK, GRID_ERR_CUDA (no device / out of memory) or GRID_ERR_UNSUPPORTED (not the warp kernel). */
+int grid_plan_autotune_candidates(const grid_plan* plan, int* out, int max_candidates);
+int grid_plan_autotune(grid_plan* plan, long long n_samples, unsigned int seed, float* results, int max_candidates,
+                       grid_stream_t stream);
+
 /* HOST out[20]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
  * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, chunk order mode,
  * polarisation split, warp groups per CTA, taps in global memory (0/1), 0. */

@@ -16,7 +16,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
     "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
-    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
+    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -47,6 +47,8 @@ _lib.grid_plan_set_traversal.argtypes = [_vp, _int, _int]
 _lib.grid_plan_set_kernel_events.argtypes = [_vp, _vp, _vp]
 _lib.grid_plan_set_chunk_order.argtypes = [_vp, _int]
 _lib.grid_plan_set_pol_split.argtypes = [_vp, _int]
+_lib.grid_plan_autotune_candidates.argtypes = [_vp, _vp, _int]
+_lib.grid_plan_autotune.argtypes = [_vp, _ll, ctypes.c_uint, _vp, _int, _vp]
 _lib.grid_plan_last_launches.argtypes = [_vp]
 _lib.grid_plan_destroy.argtypes = [_vp]
 _lib.grid_plan_destroy.restype = None
@@ -140,6 +142,22 @@ class GridPlan:
 
     def set_chunk_order(self, mode=-1):
         _check(_lib.grid_plan_set_chunk_order(self._h, mode), "grid_plan_set_chunk_order")
+
+    def autotune_candidates(self):
+        """grid_plan_autotune_candidates: list of (cu, cv, pol_split) blocks that fit this plan, the current one first."""
+        out = (ctypes.c_int * (3 * 32))()
+        n = _lib.grid_plan_autotune_candidates(self._h, out, 32)
+        if n < 0:
+            raise GridError(n, "grid_plan_autotune_candidates")
+        return [(out[3 * k], out[3 * k + 1], out[3 * k + 2]) for k in range(n)]
+
+    def autotune(self, n_samples=0, seed=1, stream=None):
+        """grid_plan_autotune: times every candidate on a synthetic data set, installs the fastest.
+        Returns [((cu, cv, pol_split), microseconds), ...] in candidate order."""
+        cands = self.autotune_candidates()
+        res = (ctypes.c_float * 32)()
+        _check(_lib.grid_plan_autotune(self._h, n_samples, seed, res, 32, _stream(stream)), "grid_plan_autotune")
+        return [(c, float(res[k])) for k, c in enumerate(cands)]
 
     def info(self) -> dict:
         out = (ctypes.c_int * 20)()

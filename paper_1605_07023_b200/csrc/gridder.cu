@@ -97,8 +97,9 @@ WarpDesc pick_warp(int logs) {
         case 3: return WarpPick<CU, CV, P, 3, PS>::get();
         case 4: return WarpPick<CU, CV, P, 4, PS>::get();
         case 5: return WarpPick<CU, CV, P, 5, PS>::get();
-        case 6: if constexpr (PS == 1 && CU * CV >= 4) return WarpPick<CU, CV, P, 6, PS>::get(); break;   // teams <= 1024 threads
-        case 7: if constexpr (PS == 1 && CU * CV >= 4) return WarpPick<CU, CV, P, 7, PS>::get(); break;   // 2 x 2 tiles of 64 x 64
+        // bins of 64 and 128 (tiles of 64 x 64): blocks of at least 8 points (teams of at most 512 threads)
+        case 6: if constexpr (PS == 1 && CU * CV >= 8) return WarpPick<CU, CV, P, 6, PS>::get(); break;
+        case 7: if constexpr (PS == 1 && CU * CV >= 8) return WarpPick<CU, CV, P, 7, PS>::get(); break;
     }
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -119,10 +120,11 @@ WarpDesc lookup_warp(int cu, int cv, int P, int logs, int ps, bool row_skip = fa
         if (cu == 2 && cv == 2 && P == 4 && ps == 1) { const WarpDesc d = pick_warp_rs<2, 2, 4, 1>(logs); if (d.fn) return d; }
     }
 #define CASE(a, b, p, s) if (cu == a && cv == b && P == p && ps == s) return pick_warp<a, b, p, s>(logs);
-    CASE(1, 1, 1, 1) CASE(2, 1, 1, 1) CASE(2, 2, 1, 1) CASE(4, 2, 1, 1) CASE(4, 4, 1, 1) CASE(8, 4, 1, 1)
-    CASE(1, 1, 2, 1) CASE(2, 2, 2, 1) CASE(4, 2, 2, 1) CASE(4, 4, 2, 1)
-    CASE(1, 1, 4, 1) CASE(2, 1, 4, 1) CASE(2, 2, 4, 1) CASE(4, 2, 4, 1)
-    CASE(2, 2, 4, 2) CASE(4, 2, 4, 2) CASE(4, 4, 4, 2) CASE(2, 1, 4, 2)
+    // the blocks the autotuner chooses from (near-square shapes); 1x1 and 2x1 never won a sweep
+    CASE(2, 2, 1, 1) CASE(4, 2, 1, 1) CASE(4, 4, 1, 1) CASE(8, 4, 1, 1)
+    CASE(2, 2, 2, 1) CASE(4, 2, 2, 1) CASE(4, 4, 2, 1)
+    CASE(2, 2, 4, 1) CASE(4, 2, 4, 1)
+    CASE(2, 2, 4, 2) CASE(4, 2, 4, 2) CASE(4, 4, 4, 2)
 #undef CASE
     return WarpDesc{nullptr, 0, 0, 0, 0, nullptr};
 }
@@ -135,8 +137,8 @@ WarpDesc pick_tg(int logs) {
 #define TGCASE(l) case l: TGBODY(l) break;
     switch (logs) {
         TGCASE(2) TGCASE(3) TGCASE(4) TGCASE(5)
-        case 6: if constexpr (CU * CV >= 4) { TGBODY(6) } break;
-        case 7: if constexpr (CU * CV >= 4) { TGBODY(7) } break;
+        case 6: if constexpr (CU * CV >= 8) { TGBODY(6) } break;
+        case 7: if constexpr (CU * CV >= 8) { TGBODY(7) } break;
     }
 #undef TGBODY
 #undef TGCASE
@@ -221,7 +223,7 @@ kernel_fn lookup_degrid(int cu, int cv, int P, int logs, bool tg = false) {
 #define CASE(a, b, p) if (cu == a && cv == b && P == p) return tg ? pick_degrid<a, b, p, true>(logs) : pick_degrid<a, b, p, false>(logs);
     CASE(2, 2, 1) CASE(4, 2, 1) CASE(4, 4, 1) CASE(8, 4, 1)
     CASE(2, 2, 2) CASE(4, 2, 2) CASE(4, 4, 2)
-    CASE(2, 1, 4) CASE(2, 2, 4) CASE(4, 2, 4)
+    CASE(2, 2, 4) CASE(4, 2, 4)
 #undef CASE
     return nullptr;
 }
@@ -475,6 +477,45 @@ QuantParams quant_params(const grid_plan* p) {
 
 }  // namespace
 
+// Autotuning: synthetic samples.  Tracks of a synthetic array: baseline b has a radius drawn
+// log-uniformly up to 0.45 N and a random orientation; time step t turns it by 4 h / 256 per step (scaled to the
+// hint's time count), channel c stretches it by up to 1.9x -- the structure of BASELINE.json's inputs, so that the
+// footprint hops per sample as it does there.  Counter-based generator (one hash per value): no state.
+__device__ __forceinline__ uint32_t tune_hash(uint32_t a, uint32_t b) {
+    uint32_t x = a * 0x9E3779B1u ^ (b + 0x7F4A7C15u) * 0x85EBCA77u;
+    x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
+    return x;
+}
+__device__ __forceinline__ float tune_unit(uint32_t a, uint32_t b) { return (tune_hash(a, b) >> 8) * (1.0f / 16777216.0f); }
+
+__global__ void __launch_bounds__(256)
+tune_fill_kernel(float* __restrict__ uvw, float2* __restrict__ vis, float* __restrict__ weights, long long n, int P,
+                 int N, int S, int W, int n_times, int n_chan, unsigned int seed) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const long long row = k / n_chan;
+    const int c = (int)(k - row * n_chan), t = (int)(row % n_times);
+    const uint32_t b = (uint32_t)(row / n_times);
+    const float rmax = 0.45f * N - S, rmin = fminf(0.02f * N, rmax);
+    const float r = rmin * __powf(rmax / rmin, tune_unit(seed, 3 * b));            // log-uniform radius
+    const float th0 = 6.2831853f * tune_unit(seed, 3 * b + 1);
+    const float th = th0 + 1.0471976f * (t - 0.5f * n_times) / (n_times > 1 ? n_times : 1);   // 60 degrees over the track
+    const float f = n_chan > 1 ? 1.0f - 0.47f * (float)(n_chan - 1 - c) / (float)(n_chan - 1) : 1.0f;   // 0.9-1.7 GHz
+    uvw[3 * k] = r * f * __cosf(th);
+    uvw[3 * k + 1] = 0.5f * r * f * __sinf(th);                                   // declination -30 degrees: v compressed
+    uvw[3 * k + 2] = W * tune_unit(seed, 3 * b + 2) * f;
+    weights[k] = 0.5f + 0.5f * tune_unit(seed + 1, (uint32_t)k);
+    for (int q = 0; q < P; ++q)
+        vis[k * P + q] = make_float2(tune_unit(seed + 2, (uint32_t)(k * P + q)) - 0.5f, tune_unit(seed + 3, (uint32_t)(k * P + q)) - 0.5f);
+}
+
+__global__ void __launch_bounds__(256) tune_taps_kernel(float2* __restrict__ kern, int rows, int S) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= rows * S) return;
+    const float d = (float)(k % S) - 0.5f * S + 0.5f;
+    kern[k] = make_float2(__expf(-4.0f * d * d / (float)(S * S)), 1e-3f * d);
+}
+
 template <int P>
 static void launch_degrid(int L, long long n, const CycRec* recs, const float* weights, const float2* kern,
                           const float2* grid, float2* out, int N, int S, cudaStream_t stream) {
@@ -586,6 +627,114 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     return GRID_OK;
 }
 
+static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs, long long n_vis, const float* vis,
+                        const float* weights, const float* conv_kernel, float* grid, cudaStream_t stream,
+                        float* degrid_out = nullptr);
+
+int grid_plan_autotune_candidates(const grid_plan* plan, int* out, int max_candidates) {
+    if (!plan || !out || max_candidates < 1) return fail(GRID_ERR_INVALID_ARG, "grid_plan_autotune_candidates: invalid argument");
+    if (plan->variant != 3) return 0;
+    static const int blocks[][2] = {{2, 2}, {4, 2}, {4, 4}, {8, 4}};
+    int n = 0;
+    auto offer = [&](int cu, int cv, int ps) {
+        if (n >= max_candidates) return;
+        for (int k = 0; k < n; ++k) if (out[3 * k] == cu && out[3 * k + 1] == cv && out[3 * k + 2] == ps) return;
+        grid_plan trial = *plan;
+        trial.cu = cu; trial.cv = cv; trial.pol_split = ps; trial.threads = 1024;
+        if (derive(&trial) != GRID_OK || trial.pol_split != ps) return;
+        out[3 * n] = cu; out[3 * n + 1] = cv; out[3 * n + 2] = ps;
+        ++n;
+    };
+    offer(plan->cu, plan->cv, plan->pol_split);                  // the current block first
+    for (int ps = 1; ps <= (plan->P == 4 ? 2 : 1); ++ps)
+        for (const auto& b : blocks) offer(b[0], b[1], ps);
+    g_err[0] = 0;
+    return n;
+}
+
+int grid_plan_autotune(grid_plan* plan, long long n_samples, unsigned int seed, float* results, int max_candidates,
+                       grid_stream_t stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!plan || n_samples < 0) return fail(GRID_ERR_INVALID_ARG, "grid_plan_autotune: invalid argument");
+    if (plan->variant != 3) return fail(GRID_ERR_UNSUPPORTED, "grid_plan_autotune: the plan does not run the warp kernel");
+    int cand[3 * 32];
+    const int n_cand = grid_plan_autotune_candidates(plan, cand, 32);
+    if (n_cand <= 0) return fail(GRID_ERR_UNSUPPORTED, "grid_plan_autotune: no candidate block fits this plan");
+    // shape of the synthetic data: the caller's layout if there is one, else single-channel tracks
+    const bool hint = plan->n_baselines > 0 && plan->n_times > 0 && plan->n_channels > 0;
+    const int n_times = hint ? plan->n_times : 256, n_chan = hint ? plan->n_channels : 1;
+    long long n = n_samples > 0 ? n_samples : (1LL << 20);
+    long long n_bl = n / ((long long)n_times * n_chan);
+    if (n_bl < 1) n_bl = 1;
+    n = n_bl * n_times * n_chan;
+    if (n >= 0x7fffffffLL) return fail(GRID_ERR_INVALID_ARG, "grid_plan_autotune: too many samples");
+
+    grid_plan t = *plan;                                         // a private plan: the caller's stays untouched until the end
+    t.n_vis = n; t.n_baselines = (int)n_bl; t.n_times = n_times; t.n_channels = n_chan;
+    t.ev_start = t.ev_stop = nullptr;
+    const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
+    const size_t kern_bytes = (size_t)plan->W * plan->O * plan->S * sizeof(float2);
+    float *d_uvw = nullptr, *d_w = nullptr, *d_grid = nullptr;
+    float2 *d_vis = nullptr, *d_kern = nullptr;
+    void* d_ws = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = GRID_OK, best = -1;
+    float best_us = 0.f;
+    auto cleanup = [&]() {
+        cudaFree(d_uvw); cudaFree(d_w); cudaFree(d_grid); cudaFree(d_vis); cudaFree(d_kern); cudaFree(d_ws);
+        if (e0) cudaEventDestroy(e0);
+        if (e1) cudaEventDestroy(e1);
+    };
+    t.workspace_bytes = grid_plan_workspace_bytes(&t);
+    if (cudaMalloc(&d_uvw, (size_t)n * 12) != cudaSuccess || cudaMalloc(&d_w, (size_t)n * 4) != cudaSuccess ||
+        cudaMalloc(&d_vis, (size_t)n * plan->P * 8) != cudaSuccess || cudaMalloc(&d_kern, kern_bytes) != cudaSuccess ||
+        cudaMalloc(&d_grid, grid_bytes) != cudaSuccess || cudaMalloc(&d_ws, t.workspace_bytes) != cudaSuccess ||
+        cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        (void)cudaGetLastError();
+        cleanup();
+        return fail(GRID_ERR_CUDA, "grid_plan_autotune: no device, or out of device memory for the synthetic data set");
+    }
+    t.workspace = d_ws;
+    tune_fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(d_uvw, d_vis, d_w, n, plan->P, plan->N, plan->S, plan->W,
+                                                                     n_times, n_chan, seed);
+    tune_taps_kernel<<<(unsigned)(((long long)plan->W * plan->O * plan->S + 255) / 256), 256, 0, stream>>>(d_kern, plan->W * plan->O, plan->S);
+    cudaMemsetAsync(d_grid, 0, grid_bytes, stream);
+    for (int k = 0; k < n_cand && rc == GRID_OK; ++k) {
+        grid_plan trial = t;
+        trial.cu = cand[3 * k]; trial.cv = cand[3 * k + 1]; trial.pol_split = cand[3 * k + 2]; trial.threads = 1024;
+        float us = -1.f;
+        if (derive(&trial) == GRID_OK) {
+            bool ok = true;
+            for (int rep = 0; rep < 2 && ok; ++rep) {            // the second run is the measurement
+                cudaEventRecord(e0, stream);
+                ok = execute_impl(&trial, d_uvw, nullptr, n, reinterpret_cast<const float*>(d_vis), d_w,
+                                  reinterpret_cast<const float*>(d_kern), d_grid, stream, nullptr) == GRID_OK;
+                cudaEventRecord(e1, stream);
+            }
+            if (ok && cudaEventSynchronize(e1) == cudaSuccess) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                us = ms * 1e3f;
+            } else if (cudaGetLastError() != cudaSuccess) {
+                rc = fail(GRID_ERR_CUDA, "grid_plan_autotune: a candidate failed on the device");
+            }
+        }
+        if (results && k < max_candidates) results[k] = us;
+        if (us > 0.f && (best < 0 || us < best_us)) { best = k; best_us = us; }
+    }
+    cudaStreamSynchronize(stream);
+    cleanup();
+    if (rc != GRID_OK) return rc;
+    if (best < 0) return fail(GRID_ERR_UNSUPPORTED, "grid_plan_autotune: no candidate ran");
+    grid_plan tuned = *plan;
+    tuned.cu = cand[3 * best]; tuned.cv = cand[3 * best + 1]; tuned.pol_split = cand[3 * best + 2]; tuned.threads = 1024;
+    if (derive(&tuned) != GRID_OK) return GRID_ERR_UNSUPPORTED;
+    *plan = tuned;
+    plan->user_tuned = 1;
+    g_err[0] = 0;
+    return GRID_OK;
+}
+
 int grid_plan_get_info(const grid_plan* plan, int* out) {
     if (!plan || !out) return fail(GRID_ERR_INVALID_ARG, "grid_plan_get_info: null argument");
     const int v[20] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
@@ -657,7 +806,7 @@ int grid_quantise(grid_plan* plan, const float* uvw, long long n, int* out, grid
 // pol split 1, team <= 32 -- the caller checks with lookup_degrid).
 static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs, long long n_vis, const float* vis,
                         const float* weights, const float* conv_kernel, float* grid, cudaStream_t stream,
-                        float* degrid_out = nullptr) {
+                        float* degrid_out) {
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
     SampleRec* recs = ext_recs ? reinterpret_cast<SampleRec*>(const_cast<void*>(ext_recs))
                                : reinterpret_cast<SampleRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);

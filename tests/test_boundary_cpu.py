@@ -128,3 +128,43 @@ def test_no_silent_scatter_fallback(binding):
     plan = binding.GridPlan(18, 13, 4, 1, 1)
     assert plan.info()["variant"] in (0, 1)
     plan.destroy()
+
+
+def test_autotune_candidates_host_logic(binding):
+    """grid_plan_autotune_candidates ("a range of coarsening factors and work-group sizes"): host logic,
+    no device.  The current (default) block comes first; every candidate is a block the plan accepts; polarisation
+    splits only with 4 polarisations; supports that do not run the warp kernel have none."""
+    for args in [(2048, 8, 8, 1, 4), (4096, 16, 8, 32, 1), (512, 7, 8, 1, 1), (4096, 32, 8, 16, 4), (4096, 64, 8, 16, 2),
+                 (4096, 128, 8, 1229, 1), (4096, 12, 4, 3, 2)]:
+        plan = binding.GridPlan(*args)
+        i = plan.info()
+        cands = plan.autotune_candidates()
+        assert cands and cands[0] == (i["cu"], i["cv"], i["pol_split"]), (args, cands)
+        assert len(set(cands)) == len(cands)
+        assert all(ps == 1 or args[4] == 4 for _, _, ps in cands)
+        for cu, cv, ps in cands:                       # each one can be installed by hand
+            trial = binding.GridPlan(*args)
+            try:                                       # split first, then the block -- or the other way round
+                if ps != trial.info()["pol_split"]:
+                    trial.set_pol_split(ps)
+                trial.set_tuning(cu=cu, cv=cv)
+            except binding.GridError:
+                trial.set_tuning(cu=cu, cv=cv)
+                trial.set_pol_split(ps)
+            assert (trial.info()["cu"], trial.info()["cv"], trial.info()["pol_split"]) == (cu, cv, ps)
+            trial.destroy()
+        plan.destroy()
+    plan = binding.GridPlan(64, 2, 4, 1, 1)           # support 2: the padded kernel, nothing to tune
+    assert plan.autotune_candidates() == []
+    plan.destroy()
+
+
+def test_autotune_needs_a_device(binding):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("device present: covered by the GPU test")
+    plan = binding.GridPlan(2048, 8, 8, 1, 4)
+    with pytest.raises(binding.GridError) as e:
+        plan.autotune(stream=0)                        # the default stream by handle: torch has no device to ask
+    assert e.value.code == binding.GRID_ERR_CUDA       # no CPU fallback, no silent success
+    plan.destroy()

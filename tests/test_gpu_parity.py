@@ -90,8 +90,8 @@ def test_every_coarsening_block(oracle_mod, cu, cv, P, S):
     assert_parity(got, ref, f"C={cu}x{cv} P={P} S={S}")
 
 
-WARP = [(1, 1, 1), (2, 1, 1), (2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (1, 1, 2), (2, 2, 2), (4, 2, 2), (4, 4, 2),
-        (1, 1, 4), (2, 1, 4), (2, 2, 4), (4, 2, 4)]
+# every instantiated block of the warp kernel (= the autotuner's candidates)
+WARP = [(2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (2, 2, 2), (4, 2, 2), (4, 4, 2), (2, 2, 4), (4, 2, 4)]
 
 
 @pytest.mark.parametrize("cu,cv,P", WARP)
@@ -115,7 +115,7 @@ def test_every_warp_block(oracle_mod, cu, cv, P, S):
         assert_parity(got, ref, f"warp C={cu}x{cv} P={P} S={S} batch={batch} {info}")
 
 
-@pytest.mark.parametrize("cu,cv", [(2, 1), (2, 2), (4, 2), (4, 4)])
+@pytest.mark.parametrize("cu,cv", [(2, 2), (4, 2), (4, 4)])
 @pytest.mark.parametrize("S", [4, 8, 16, 32])
 def test_warp_block_pol_split(oracle_mod, cu, cv, S):
     # 4 polarisations spread over lane pairs (grid_plan_set_pol_split): same result as the oracle
@@ -194,7 +194,7 @@ def test_sorted_chunk_queue(oracle_mod, name, ps, mode):
     assert_parity(got, ref, f"{name} sorted queue mode={mode}")
 
 
-@pytest.mark.parametrize("cu,cv,P,W", [(8, 4, 1, 2), (4, 4, 1, 2), (4, 2, 1, 3), (2, 2, 1, 2), (4, 2, 4, 2), (4, 4, 2, 2), (4, 2, 2, 2),
+@pytest.mark.parametrize("cu,cv,P,W", [(8, 4, 1, 2), (4, 4, 1, 2), (4, 2, 1, 3), (4, 2, 4, 2), (4, 4, 2, 2), (4, 2, 2, 2),
                                        (8, 4, 1, 40), (4, 2, 4, 40)])
 @pytest.mark.parametrize("mode", [0, 1])
 def test_support_64(oracle_mod, cu, cv, P, W, mode):
@@ -220,7 +220,7 @@ def test_support_64(oracle_mod, cu, cv, P, W, mode):
     assert_parity(got, ref, f"S=64 C={cu}x{cv} P={P} W={W} mode={mode} {info}")
 
 
-@pytest.mark.parametrize("cu,cv,P,W", [(8, 4, 1, 2), (4, 4, 1, 2), (4, 2, 4, 2), (4, 4, 2, 2), (2, 2, 1, 2), (8, 4, 1, 40), (4, 2, 4, 40)])
+@pytest.mark.parametrize("cu,cv,P,W", [(8, 4, 1, 2), (4, 4, 1, 2), (4, 2, 4, 2), (4, 4, 2, 2), (8, 4, 1, 40), (4, 2, 4, 40)])
 @pytest.mark.parametrize("mode", [0, 1])
 def test_support_128_tiled(oracle_mod, cu, cv, P, W, mode):
     # S = 128 (the paper's largest bin): the bin is split into 2 x 2 tiles of 64 x 64 positions, one team per
@@ -359,3 +359,31 @@ def test_repeat_execute_accumulates(oracle_mod):
     torch.cuda.synchronize()
     plan.destroy()
     assert_parity(grid.cpu().numpy(), 3 * ref, "3x execute")
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg0"])
+def test_autotuned_plan_stays_in_parity(oracle_mod, name):
+    # grid_plan_autotune: times every candidate block on a synthetic data set, installs the fastest;
+    # the tuned plan must give the oracle's grid, and the result table must cover every candidate
+    import torch
+    from paper_1605_07023_b200 import binding
+    cfg = synth.shrink(synth.get_config(name), n_ant=12, n_times=40, n_chan=16, grid_size=512)
+    wl = synth.make_workload(cfg)
+    N, S, O, W, P = cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol
+    ref = oracle_mod.grid(N, S, O, W, P, wl.uvw, wl.vis, wl.weights, wl.kernel)
+    dev = torch.device("cuda:0")
+    plan = binding.GridPlan(N, S, O, W, P)
+    plan.set_samples(cfg.n_vis)
+    plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    cands = plan.autotune_candidates()
+    table = plan.autotune(n_samples=1 << 17, seed=3)
+    assert [c for c, _ in table] == cands and all(us > 0 for _, us in table), table
+    i = plan.info()
+    best = min(table, key=lambda e: e[1])[0]
+    assert (i["cu"], i["cv"], i["pol_split"]) == best
+    plan.allocate_workspace(dev)
+    grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+    plan.execute(*(torch.from_numpy(a).to(dev) for a in (wl.uvw, wl.vis, wl.weights, wl.kernel)), grid)
+    torch.cuda.synchronize()
+    plan.destroy()
+    assert_parity(grid.cpu().numpy(), ref, f"autotuned {name}: {best} of {table}")

@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--no-per-config", action="store_true",
                     help="skip the per_config table (every BASELINE.json config, device-resident, with an oracle row band)")
     ap.add_argument("--per-config-steps", type=int, default=5)
+    ap.add_argument("--autotune", action="store_true",
+                    help="per_config: run grid_plan_autotune on every config first (PAPER.md:101) and report the table of "
+                         "candidate blocks with their times next to the plan's default")
     return ap.parse_args()
 
 
@@ -230,7 +233,7 @@ def reduce_over_ranks(times_ms, units, device, world):
 ALL_CONFIGS = ["cfg0", "cfg1", "cfg2", "cfg3"] + [f"cfg4_S{s}_P{p}" for s in (4, 8, 16, 32) for p in (1, 4)]
 
 
-def measure_config(name, steps, warmup, dev, oracle_band=True):
+def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False):
     """One BASELINE.json config, device-resident: K timed grid_execute calls (CUDA events on the launching
     stream, L2 scrubbed between steps when the inputs could stay in it), the hot kernel's own time, and the
     rel-L2 / max-abs error of one band of grid rows against the float64 oracle (row-restricted mode)."""
@@ -244,6 +247,12 @@ def measure_config(name, steps, warmup, dev, oracle_band=True):
     plan = binding.GridPlan(N, S, O, W, P)
     plan.set_samples(cfg.n_vis)
     plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    tuned = None
+    if autotune:                                               # time every candidate block, keep the fastest
+        default = plan.info()
+        table = plan.autotune(n_samples=1 << 21, seed=1)
+        tuned = {"default": "%dx%d ps%d" % (default["cu"], default["cv"], default["pol_split"]),
+                 "candidates_us": {"%dx%d ps%d" % c: round(us, 1) for c, us in table}}
     plan.allocate_workspace(dev)
     info = plan.info()
     q = plan.quantise(d_uvw)
@@ -294,7 +303,7 @@ def measure_config(name, steps, warmup, dev, oracle_band=True):
                          "kernel_ms": kernel_ms, "kernel": kernel_template_name(info, P, S)},
             "block": "%dx%d, pol split %d, %d threads, batch %d" % (info["cu"], info["cv"], info["pol_split"],
                                                                     info["threads_per_cta"], info["batch"]),
-            "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err}
+            "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err, "autotune": tuned}
 
 
 def run_wstack(args):
@@ -580,7 +589,7 @@ def run_ours(args):
             plan.destroy()
             del d_uvw, d_vis, d_wts, grid, h_uvw, h_vis, h_wts
             torch.cuda.empty_cache()
-            line["per_config"] = [measure_config(n, args.per_config_steps, 3, dev) for n in ALL_CONFIGS]
+            line["per_config"] = [measure_config(n, args.per_config_steps, 3, dev, autotune=args.autotune) for n in ALL_CONFIGS]
         print(json.dumps(line), flush=True)
     plan.destroy()
     if world > 1:

@@ -205,6 +205,13 @@ int grid_plan_get_info(const grid_plan* plan, int* out);
  * quantise pass a1 lies outside the pair).  NULL, NULL clears.  Nothing is synchronised. */
 int grid_plan_set_kernel_events(grid_plan* plan, void* ev_start, void* ev_stop);
 
+/* Checked build only (nvcc -DGRIDB200_CHECK, tests/test_gpu_checked_build.py; compute-sanitizer is closed on the
+ * measurement pool): the warp kernel tests every global address it forms and every shared-memory slot it indexes
+ * against its bounds, counts violations and suppresses the access.  HOST out[8] = violations since the last call
+ * that reset the plan's queue: grid cell, sample index, raw slot, cooked slot, tap offset, degrid output index, 0, 0.
+ * Synchronises `stream`.  The shipped library compiles the tests away and always reports zeros. */
+int grid_plan_debug_counters(grid_plan* plan, unsigned int* out, grid_stream_t stream);
+
 /* Kernel launches enqueued by the last grid_execute on this plan (for bench.py's gpu_launches). */
 int grid_plan_last_launches(const grid_plan* plan);
 

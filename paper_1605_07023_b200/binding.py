@@ -9,14 +9,15 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgridb200.so")
+# GRIDB200_LIB: another build of the same library (the bounds-checked one of tests/test_gpu_checked_build.py)
+LIB_PATH = os.environ.get("GRIDB200_LIB") or os.path.join(_HERE, "libgridb200.so")
 
 GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STATE = 0, -1, -2, -3, -4
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
     "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
-    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_destroy", "grid_last_error",
+    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_debug_counters", "grid_plan_destroy", "grid_last_error",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -50,6 +51,7 @@ _lib.grid_plan_set_pol_split.argtypes = [_vp, _int]
 _lib.grid_plan_autotune_candidates.argtypes = [_vp, _vp, _int]
 _lib.grid_plan_autotune.argtypes = [_vp, _ll, ctypes.c_uint, _vp, _int, _vp]
 _lib.grid_plan_last_launches.argtypes = [_vp]
+_lib.grid_plan_debug_counters.argtypes = [_vp, _vp, _vp]
 _lib.grid_plan_destroy.argtypes = [_vp]
 _lib.grid_plan_destroy.restype = None
 _lib.grid_last_error.restype = ctypes.c_char_p
@@ -169,6 +171,12 @@ class GridPlan:
         a = ev_start.cuda_event if ev_start is not None else None
         b = ev_stop.cuda_event if ev_stop is not None else None
         _check(_lib.grid_plan_set_kernel_events(self._h, a, b), "grid_plan_set_kernel_events")
+
+    def debug_counters(self, stream=None):
+        """grid_plan_debug_counters: bounds violations counted by a -DGRIDB200_CHECK build (zeros otherwise)."""
+        out = (ctypes.c_uint * 8)()
+        _check(_lib.grid_plan_debug_counters(self._h, out, _stream(stream)), "grid_plan_debug_counters")
+        return list(out)
 
     def last_launches(self) -> int:
         return int(_lib.grid_plan_last_launches(self._h))

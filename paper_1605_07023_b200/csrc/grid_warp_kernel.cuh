@@ -120,6 +120,18 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // each holding PT = P/PS of them.  With P = 4, PS = 2 the two 16-byte atomics that make up one
 // 32-byte grid point come from neighbouring lanes of ONE instruction and reach the L2 as one sector
 // operation instead of two -- the L2's atomic sector rate is the second bound of this kernel.
+// Checked build (-DGRIDB200_CHECK; compute-sanitizer is closed on the measurement pool): every global address the
+// kernel forms and every shared-memory slot it indexes is tested against its bounds; violations are counted in
+// gp.counters[kCheckBase + code] (read back with grid_plan_debug_counters) and the access is suppressed.  The
+// shipped library compiles these tests away.
+static constexpr int kCheckBase = 40;            // counters[40..47]
+enum { kChkGridCell = 0, kChkSampleIndex = 1, kChkRawSlot = 2, kChkCookedSlot = 3, kChkTapOffset = 4, kChkOutIndex = 5 };
+#ifdef GRIDB200_CHECK
+#define GRIDB200_CHK(cond, code) ((cond) ? true : (atomicAdd(gp.counters + kCheckBase + (code), 1u), false))
+#else
+#define GRIDB200_CHK(cond, code) true
+#endif
+
 template <int CU, int CV, int P, int LOGS, int PS = 1>
 struct WarpKernelTraits {
     static_assert(P % PS == 0, "polarisations must divide evenly over the split");
@@ -279,6 +291,7 @@ grid_warp_kernel(const GridParams gp) {
 
     // a8: one grid point, all polarisations: atomic add, then clear
     auto flush_point = [&](float2 (&v)[PT], uint32_t cell) {
+        if (!GRIDB200_CHK(cell < (uint32_t)gp.N * (uint32_t)gp.N, kChkGridCell)) { clear_point(v); return; }
         float* p = gridp + (size_t)cell * (2 * P) + half * (2 * PT);
         if constexpr (PT == 4) {
             red_add_v4(p, v[0].x, v[0].y, v[1].x, v[1].y);
@@ -294,6 +307,7 @@ grid_warp_kernel(const GridParams gp) {
     // Same, but the atomic adds are predicated: used in the row pass for points whose column has
     // just been flushed (their accumulators are zero; skipping saves the L2 traffic, not a branch).
     auto flush_point_if = [&](float2 (&v)[PT], uint32_t cell, uint32_t skip) {
+        if (!GRIDB200_CHK(skip || cell < (uint32_t)gp.N * (uint32_t)gp.N, kChkGridCell)) { clear_point(v); return; }
         float* p = gridp + (size_t)cell * (2 * P) + half * (2 * PT);
         if constexpr (PT == 4) {
             asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.u32 q, %9, 0;\n\t"
@@ -417,6 +431,7 @@ grid_warp_kernel(const GridParams gp) {
             const WarpChunk cg = {g4.x, g4.y, g4.z, g4.w};
             if (k >= count_of(cg, b)) continue;
             const uint32_t g = sample_of(cg, (b << bshift) + k);
+            if (!GRIDB200_CHK(g < n_vis32, kChkSampleIndex) || !GRIDB200_CHK(kk < slots && st < 2, kChkRawSlot)) continue;
             if (gp.rec16) {
                 cp_async_16(rrec + kk, reinterpret_cast<const uint4*>(gp.recs) + g);
             } else {
@@ -445,6 +460,7 @@ grid_warp_kernel(const GridParams gp) {
             const WarpChunk cg = {g4.x, g4.y, g4.z, g4.w};
             const int cnt = count_of(cg, b);
             const int ck = t * BP + k;                 // slot in the cooked arrays
+            if (!GRIDB200_CHK(ck < cslots && t < TPG, kChkCookedSlot)) continue;
             uint4 c = make_uint4(0u, 0u, 0u, 0u);
             if constexpr (W64) cmask[ck] = make_uint4(0u, 0u, 0u, 0u);
             uint32_t code = 0xffffffffu;               // DEGRID: where the result goes; all ones = no sample
@@ -692,6 +708,10 @@ grid_warp_kernel(const GridParams gp) {
                     tv = reinterpret_cast<const float2*>(my_tv + c.z);
                 }
                 c = *++rp;                             // next sample's record
+                if constexpr (!TG) {                   // the taps this thread is about to read lie inside the table
+                    (void)GRIDB200_CHK(tu >= staps && tu + (CU - 1) * DU < staps + (size_t)gp.n_rows * ROW &&
+                                       tv >= staps && tv + (CV - 1) * DV < staps + (size_t)gp.n_rows * ROW, kChkTapOffset);
+                }
                 float2 gu[CU], gv[CV], v[PT];
 #pragma unroll
                 for (int a = 0; a < CU; ++a) gu[a] = tu[a * DU];
@@ -755,7 +775,7 @@ grid_warp_kernel(const GridParams gp) {
                     constexpr int LOGT = WT >= 32 ? 5 : WT >= 16 ? 4 : WT >= 8 ? 3 : WT >= 4 ? 2 : WT >= 2 ? 1 : 0;
                     constexpr int WLAST = (W0 >> LOGT) > 1 ? (W0 >> LOGT) : 1;      // floats left per lane
                     const uint32_t code = __float_as_uint(meta.y);
-                    if ((lt & dup & 31) == 0 && code != 0xffffffffu) {
+                    if ((lt & dup & 31) == 0 && code != 0xffffffffu && GRIDB200_CHK((code & 0x7fffffffu) < n_vis32, kChkOutIndex)) {
                         float* o = reinterpret_cast<float*>(gp.vis_out + (size_t)(code & 0x7fffffffu) * P) + first;
                         const float w = meta.x;
                         if constexpr (GW > 1 || NT > 1) {

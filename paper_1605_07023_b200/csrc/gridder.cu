@@ -781,6 +781,17 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode) {
 
 int grid_plan_last_launches(const grid_plan* plan) { return plan ? plan->last_launches : 0; }
 
+int grid_plan_debug_counters(grid_plan* plan, unsigned int* out, grid_stream_t stream) {
+    if (!plan || !out) return fail(GRID_ERR_INVALID_ARG, "grid_plan_debug_counters: null argument");
+    memset(out, 0, 8 * sizeof(unsigned int));
+    if (!plan->workspace) return GRID_OK;
+    const unsigned int* src = reinterpret_cast<const unsigned int*>(plan->workspace) + kCheckBase;
+    if (cudaMemcpyAsync(out, src, 8 * sizeof(unsigned int), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||
+        cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+        return fail(GRID_ERR_CUDA, "grid_plan_debug_counters: %s", cudaGetErrorString(cudaGetLastError()));
+    return GRID_OK;
+}
+
 int grid_plan_set_kernel_events(grid_plan* plan, void* ev_start, void* ev_stop) {
     if (!plan || ((ev_start == nullptr) != (ev_stop == nullptr)))
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_kernel_events: pass two events or two NULLs");

@@ -192,16 +192,19 @@ def ncu_traffic(workload, kernel_name):
     return e.get("dram_bytes_per_launch")
 
 
-def kernel_template_name(info, P, S, op="grid"):
+def kernel_template_name(info, P, S, op="grid", N=None):
     """Name of the launched hot kernel as ncu prints it (template arguments from the plan)."""
     if info["variant"] == 0:
         return "grid_scatter_kernel<%d>" % P
     if info["variant"] == 1:
         return "grid_coarsened_kernel<%d, %d, %d>" % (info["cu"], info["cv"], P)
-    logs = S.bit_length() - 1
-    return "grid_warp_kernel<%d, %d, %d, %d, %d, %d, %d, %d>" % (
+    logs = (S - 1).bit_length()                    # supports that are not powers of two run zero-padded to the next one
+    # last argument: the row-skip instantiation, used for 4-pol 2x2 blocks on grids beyond 1 GB (gridder.cu)
+    rs = 1 if (op == "grid" and N is not None and N * N * P * 8 > (1 << 30) and (info["cu"], info["cv"], P) == (2, 2, 4)
+               and logs <= 4) else 0
+    return "grid_warp_kernel<%d, %d, %d, %d, %d, %d, %d, %d, %d>" % (
         info["cu"], info["cv"], P, logs, info["pol_split"], 1 if op == "degrid" else 0,
-        info["taps_global"], 1 if op == "dense" else 0)
+        info["taps_global"], 1 if op == "dense" else 0, rs)
 
 
 def parse_tuning(text):
@@ -300,7 +303,7 @@ def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False):
             "updates_per_step": updates, "steps": steps, "ms_per_step": ms, "value": rate, "unit": "updates/s",
             "pct_fp32_roofline": 100.0 * rate * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
             "roofline": {"bound": "alu", "frac": updates * FLOPS_PER_UPDATE / (kernel_ms * 1e-3) / (PEAK_FP32_TFLOPS * 1e12),
-                         "kernel_ms": kernel_ms, "kernel": kernel_template_name(info, P, S)},
+                         "kernel_ms": kernel_ms, "kernel": kernel_template_name(info, P, S, "grid", N)},
             "block": "%dx%d, pol split %d, %d threads, batch %d" % (info["cu"], info["cv"], info["pol_split"],
                                                                     info["threads_per_cta"], info["batch"]),
             "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err, "autotune": tuned}
@@ -382,7 +385,7 @@ def run_wstack(args):
         upd = w["n_c"] * S * S * P
         per_slice.append({"slice": i, "n_vis": w["n"], "n_compressed": w["n_c"], "kernel_ms": kms,
                           "pct_fp32_roofline_kernel": 100.0 * upd * FLOPS_PER_UPDATE / (kms * 1e-3) / (PEAK_FP32_TFLOPS * 1e12),
-                          "kernel": kernel_template_name(info, P, S)})
+                          "kernel": kernel_template_name(info, P, S, "grid", N)})
         w["plan"].set_kernel_events(None, None)
     big = max(range(len(work)), key=lambda i: work[i]["n_c"])
     achieved = work[big]["n_c"] * S * S * P * FLOPS_PER_UPDATE / (per_slice[big]["kernel_ms"] * 1e-3) / 1e12
@@ -445,7 +448,7 @@ def run_ours(args):
         plan.set_tuning(**tuning)
     plan.allocate_workspace(dev)
     info = plan.info()
-    kernel_name = kernel_template_name(info, P, S, args.op)
+    kernel_name = kernel_template_name(info, P, S, args.op, N)
 
     # number of valid samples (for the metric) from the library's own quantise pass
     q = plan.quantise(d_uvw)

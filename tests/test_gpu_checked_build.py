@@ -60,7 +60,9 @@ for S, P, O, W, extra in cases:
         out.append(dict(S=S, P=P, W=W, mode=mode, variant=plan.info()["variant"], grid_counters=c1, degrid_counters=c2,
                         rel=float(rel), max_abs=float(mx), degrid_rel=drel))
         plan.destroy()
-print("RESULT " + json.dumps(out))
+print("RESULT " + json.dumps(out), flush=True)
+import os
+os._exit(0)            # skip interpreter teardown (ctypes handles of a second copy of the library)
 '''
 
 
@@ -70,8 +72,9 @@ def test_checked_build_reports_no_violation():
     lib = entry.build_checked()
     env = dict(os.environ, GRIDB200_LIB=lib)
     r = subprocess.run([sys.executable, "-c", CHILD, ROOT], env=env, capture_output=True, text=True, timeout=1200)
-    assert r.returncode == 0, r.stderr[-2000:]
-    line = [l for l in r.stdout.splitlines() if l.startswith("RESULT ")][-1]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("RESULT ")]
+    assert r.returncode == 0 and lines, (r.returncode, r.stdout[-1000:], r.stderr[-3000:])
+    line = lines[-1]
     res = json.loads(line[len("RESULT "):])
     assert len(res) == 18
     for e in res:

@@ -2,8 +2,9 @@
 //
 // The paper hands out fixed-size chunks of baseline-ordered samples; which chunk a
 // work-group takes next does not change the result.  On B200 the atomic flushes of a grid that does
-// not fit the 126 MB L2 are bound by DRAM sector fetches (profiles/r1_ncu_full_v3_cfg3.txt: 35 GB of
-// DRAM traffic for a 2.1 GB grid), because the ~7000 chunks in flight lie all over the uv plane.
+// not fit the 126 MB L2 cost DRAM sector fetches (round 1, before this ordering existed: 35 GB of DRAM traffic
+// per launch for cfg3's 2.1 GB grid; with it 8-12 GB, profiles/r2_ncu_full_cfg3.txt), because the ~7000 chunks in
+// flight lie all over the uv plane.
 // These three small kernels sort the chunk ids by the coarse grid tile of the chunk's first sample
 // (counting sort: histogram, scan, scatter), so that chunks in flight together touch a few
 // neighbouring tiles.  Inputs are the quantised records written by the a1 pass.

@@ -44,12 +44,12 @@ struct grid_plan {
     int traversal, time_block;      // -1 auto / 0 channel-innermost / 1 time-innermost; Tc
     // derived
     int bin_u, bin_v, row_u, row_v, nbx, nby, team_threads, teams_per_cta, smem_bytes;
-    int groups_per_cta, queue_teams;
+    int groups_per_cta, queue_teams;      // variant 3: warp groups per CTA; teams per queue entry (all variants)
     int dense;                            // internal (grid_execute_dense): non-separable table, read from global memory; 2: one per polarisation
     int taps_global;                      // variant 3: tap table read from global memory (too large for shared)
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
-    int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on      // variant 3: warp groups per CTA; teams per queue entry (all variants)
+    int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on
     int n_sm, max_smem;
     int last_launches;
     int user_tuned;                       // set_tuning / set_pol_split was called: set_samples keeps the block

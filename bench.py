@@ -536,21 +536,52 @@ def run_ours(args):
         e_steps = max(3, min(args.steps, 10))
         h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4
         d2h = h_grid.numel() * 8
+        # The user's call sequence for host data: the samples go to the device in K groups of whole baselines on a
+        # copy stream while the previous group is gridded (grid_execute accumulates, so K calls on K sub-ranges give the
+        # same grid); the grid comes back once per step.  Everything below is inside the timed region.
+        K = 8 if (cfg.n_baselines >= 64 and h2d > (256 << 20)) else 1      # small inputs: one copy, one call
+        per_bl = cfg.n_times * cfg.n_chan
+        cuts = [round(i * cfg.n_baselines / K) for i in range(K + 1)]
+        parts = []
+        for i in range(K):
+            nb = cuts[i + 1] - cuts[i]
+            sub = binding.GridPlan(N, S, O, W, P)
+            sub.set_samples(nb * per_bl)
+            sub.set_layout(nb, cfg.n_times, cfg.n_chan)
+            sub.allocate_workspace(dev)
+            lo, hi = cuts[i] * per_bl, cuts[i + 1] * per_bl
+            parts.append({"plan": sub, "lo": lo, "hi": hi, "copied": torch.cuda.Event(), "done": torch.cuda.Event()})
+        copy_stream = torch.cuda.Stream(device=dev)
+
+        def e2e_step():
+            for part in parts:
+                lo, hi = part["lo"], part["hi"]
+                copy_stream.wait_event(part["done"])               # the previous step's gridding of this range
+                with torch.cuda.stream(copy_stream):
+                    d_uvw[lo:hi].copy_(h_uvw[lo:hi], non_blocking=True)
+                    d_vis[lo:hi].copy_(h_vis[lo:hi], non_blocking=True)
+                    d_wts[lo:hi].copy_(h_wts[lo:hi], non_blocking=True)
+                    part["copied"].record(copy_stream)
+                stream.wait_event(part["copied"])
+                part["plan"].execute(d_uvw[lo:hi], d_vis[lo:hi], d_wts[lo:hi], d_kern, grid)
+                part["done"].record(stream)
+            h_grid.copy_(grid, non_blocking=True)
+
+        for part in parts:
+            part["done"].record(stream)
         for _ in range(2):
-            d_uvw.copy_(h_uvw, non_blocking=True)
+            e2e_step()
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(e_steps):
-            d_uvw.copy_(h_uvw, non_blocking=True)
-            d_vis.copy_(h_vis, non_blocking=True)
-            d_wts.copy_(h_wts, non_blocking=True)
-            plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
-            h_grid.copy_(grid, non_blocking=True)
+            e2e_step()
         e1.record(stream)
         barrier()
         e2e_ms = e0.elapsed_time(e1)
-        e2e = {"ms": e2e_ms, "steps": e_steps, "h2d": h2d, "d2h": d2h}
+        e2e = {"ms": e2e_ms, "steps": e_steps, "h2d": h2d, "d2h": d2h, "groups": K}
+        for part in parts:
+            part["plan"].destroy()
 
     (elapsed_ms, e2e_step_ms, kernel_ms), total_updates_per_step = reduce_over_ranks(
         [elapsed_ms, e2e["ms"] / e2e["steps"] if e2e else 0.0, kernel_ms], updates_per_step, dev, world)
@@ -579,7 +610,9 @@ def run_ours(args):
         if e2e:
             line["e2e"] = {"value": total_updates_per_step / (e2e_step_ms * 1e-3), "unit": "updates/s",
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
-                           "ms_per_step": e2e_step_ms}
+                           "ms_per_step": e2e_step_ms,
+                           "how": "%d groups of baselines: pinned host -> device copies on a copy stream overlapped with "
+                                  "grid_execute of the previous group; grid read back once per step" % e2e["groups"]}
         if not args.no_cpu_baseline and world >= 1:
             stride = 4 if cfg.n_baselines >= 64 else 1
             v, dt, upd, n_bl, cores = time_oracle(wl, stride)

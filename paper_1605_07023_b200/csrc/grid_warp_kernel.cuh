@@ -346,7 +346,6 @@ grid_warp_kernel(const GridParams gp) {
                                : (gp.chunk + B - 1) >> bshift;
 
     const uint32_t n_vis32 = (uint32_t)gp.n_vis, n_chan = (uint32_t)gp.n_chan;
-    const uint64_t stream_policy = l2_evict_first_policy();
     const uint32_t tc = (uint32_t)gp.tc;               // a power of two (grid_plan_set_traversal)
     const int tshift = 31 - __clz((int)(tc > 0 ? tc : 1));
 
@@ -436,6 +435,7 @@ grid_warp_kernel(const GridParams gp) {
     // record {origin, tap rows, weight} (8 bytes + a separate weight for pre-quantised, compressed input)
     // and its visibilities
     auto issue = [&](int par, int b, int st) {
+        const uint64_t stream_policy = l2_evict_first_policy();       // made where it is used: a short-lived uniform value
         unsigned char* rs = rbase + (size_t)st * rstage;
         float2* rvis = reinterpret_cast<float2*>(rs);
         uint4* rrec = reinterpret_cast<uint4*>(rs + (size_t)slots * 8 * P);

@@ -113,19 +113,9 @@ __device__ __forceinline__ void cp_async_8(void* dst, const void* src) {
 __device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
-// The same with an L2 eviction hint: the samples are read once and should not displace the grid, whose cells are
-// hit by atomics again and again (cfg1: a 134 MB grid against 126 MB of L2 and 1.6 GB of streamed input).
-__device__ __forceinline__ uint64_t l2_evict_first_policy() {
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void cp_async_8_hint(void* dst, const void* src, uint64_t pol) {
-    asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void cp_async_16_hint(void* dst, const void* src, uint64_t pol) {
-    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "l"(pol) : "memory");
-}
+// (An L2 evict-first hint on these copies -- cp.async ... .L2::cache_hint with a createpolicy value or with the fixed
+//  encoding -- gained 1.5-3.5 % on every config and was taken out again: with it some kernels raised "illegal
+//  instruction" on some boxes / driver versions and not on others, with the same binary; profiles/r2_experiments.md.)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -435,7 +425,6 @@ grid_warp_kernel(const GridParams gp) {
     // record {origin, tap rows, weight} (8 bytes + a separate weight for pre-quantised, compressed input)
     // and its visibilities
     auto issue = [&](int par, int b, int st) {
-        const uint64_t stream_policy = l2_evict_first_policy();       // made where it is used: a short-lived uniform value
         unsigned char* rs = rbase + (size_t)st * rstage;
         float2* rvis = reinterpret_cast<float2*>(rs);
         uint4* rrec = reinterpret_cast<uint4*>(rs + (size_t)slots * 8 * P);
@@ -447,16 +436,16 @@ grid_warp_kernel(const GridParams gp) {
             const uint32_t g = sample_of(cg, (b << bshift) + k);
             if (!GRIDB200_CHK(g < n_vis32, kChkSampleIndex) || !GRIDB200_CHK(kk < slots && st < 2, kChkRawSlot)) continue;
             if (gp.rec16) {
-                cp_async_16_hint(rrec + kk, reinterpret_cast<const uint4*>(gp.recs) + g, stream_policy);
+                cp_async_16(rrec + kk, reinterpret_cast<const uint4*>(gp.recs) + g);
             } else {
                 cp_async_8(rrec + kk, reinterpret_cast<const CycRec*>(gp.recs) + g);
                 if (gp.weights) cp_async_4(&rrec[kk].z, gp.weights + g);   // null: pre-weighted (compressed) input
             }
             if constexpr (DEGRID) {
-            } else if constexpr (P == 1) cp_async_8_hint(rvis + kk, gp.vis + g, stream_policy);
+            } else if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + g);
             else {
 #pragma unroll
-                for (int q = 0; q < P; q += 2) cp_async_16_hint(rvis + (size_t)kk * P + q, gp.vis + (size_t)g * P + q, stream_policy);
+                for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + (size_t)g * P + q);
             }
         }
         cp_async_commit();

@@ -73,6 +73,23 @@ int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes);
 int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                  const float* conv_kernel, float* grid, grid_stream_t stream);
 
+/* grid_execute without a caller-provided workspace and without any allocation: for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The workspace of the
+ * call -- chunk queue and statistics, quantised records, chunk order, tap table copy; what grid_plan_set_workspace
+ * otherwise supplies -- lives in ONE array of GRID_STATIC_SCRATCH_BYTES in the library's device image (every GPU that
+ * loads the library holds it until the process exits).  Same arguments, same result and same kernels as
+ * grid_execute; grid_plan_set_workspace need not have been called and is ignored.
+ *   - Returns GRID_ERR_UNSUPPORTED, with the sizes in grid_last_error(), when grid_plan_workspace_bytes(plan) exceeds
+ *     GRID_STATIC_SCRATCH_BYTES (20 MiB: about 1.2 million samples per call; fewer when the tap table has to be
+ *     copied to global memory).  Grid larger inputs in several calls: the grid is accumulated into.
+ *   - Calls no cudaMalloc / cudaFree or allocating library routine (one cudaGetSymbolAddress per device on first use).
+ *   - The array is shared by every plan and every call on a device and keeps the last call's contents; the call
+ *     clears the part that must start at zero (queue, statistics, order bins) on `stream` before use.  Two calls
+ *     that overlap on the GPU (different streams, no ordering between them) RACE on it: serialise them. */
+#define GRID_STATIC_SCRATCH_BYTES (20u << 20)
+int grid_execute_static(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                        const float* conv_kernel, float* grid, grid_stream_t stream);
+
 /* Compression, the step before the path ("merge adjacent visibilities with identical
  * oversampled position", done as a pre-process and reused for every major cycle; PAPER.md:91 lists what a
  * compressed sample carries).  Runs a1 and merges every run of consecutive samples with equal

@@ -16,7 +16,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
-    "grid_plan_set_workspace", "grid_execute", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
+    "grid_plan_set_workspace", "grid_execute", "grid_execute_static", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
     "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_debug_counters", "grid_plan_destroy", "grid_last_error",
 )
 
@@ -35,6 +35,7 @@ _lib.grid_plan_workspace_bytes.argtypes = [_vp]
 _lib.grid_plan_workspace_bytes.restype = _sz
 _lib.grid_plan_set_workspace.argtypes = [_vp, _vp, _sz]
 _lib.grid_execute.argtypes = [_vp] * 7
+_lib.grid_execute_static.argtypes = [_vp] * 7
 _lib.grid_quantise.argtypes = [_vp, _vp, _ll, _vp, _vp]
 _lib.grid_compress.argtypes = [_vp] * 8
 _lib.grid_execute_dense.argtypes = [_vp] * 7
@@ -212,6 +213,19 @@ class GridPlan:
                                _ptr(conv_kernel, torch.complex64, "conv_kernel"),
                                _ptr(grid, torch.complex64, "grid"), _stream(stream))
         _check(rc, "grid_execute")
+
+    def execute_static(self, uvw, vis, weights, conv_kernel, grid, stream=None):
+        """grid_execute_static: grid_execute with the workspace in the library's static device array -- no allocation;
+        at most GRID_STATIC_SCRATCH_BYTES (20 MiB, about 1.2 million samples) per call; calls must not overlap on the GPU."""
+        import torch
+        self._check_samples(uvw, vis, weights, grid)
+        if conv_kernel.numel() != self.n_wplanes * self.oversample * self.support:
+            raise ValueError("conv_kernel must be [n_wplanes][oversample][support]")
+        rc = _lib.grid_execute_static(self._h, _ptr(uvw, torch.float32, "uvw"), _ptr(vis, torch.complex64, "vis"),
+                                      _ptr(weights, torch.float32, "weights"),
+                                      _ptr(conv_kernel, torch.complex64, "conv_kernel"),
+                                      _ptr(grid, torch.complex64, "grid"), _stream(stream))
+        _check(rc, "grid_execute_static")
 
     def execute_dense(self, uvw, vis, weights, conv_kernel_2d, grid, stream=None):
         """grid_execute_dense: conv_kernel_2d complex64 [W][O][O][S][S] (plane, sv, su, row, column)."""

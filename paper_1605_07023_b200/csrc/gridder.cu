@@ -993,6 +993,60 @@ int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const floa
     return execute_impl(plan, uvw, nullptr, plan->n_vis, vis, weights, conv_kernel, grid, (cudaStream_t)stream);
 }
 
+// ---- grid_execute_static: the call's workspace in the library's own device image (no allocation anywhere).
+// In host code `g_static_scratch` is a host-side stand-in for the symbol, NOT a device address: the device address
+// is asked for once per device (cudaGetSymbolAddress, with that device current) and that pointer goes to the kernels.
+static __device__ __align__(256) unsigned char g_static_scratch[GRID_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_pointer(void** out) {
+    constexpr int kMaxDevices = 64;
+    static void* ptrs[kMaxDevices] = {nullptr};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        (void)cudaGetLastError();
+        return fail(GRID_ERR_CUDA, "grid_execute_static: no current CUDA device (the gridder has no CPU fallback)");
+    }
+    if (!ptrs[dev]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            return fail(GRID_ERR_CUDA, "grid_execute_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+        }
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return GRID_OK;
+}
+
+int grid_execute_static(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
+                        const float* conv_kernel, float* grid, grid_stream_t stream) {
+    if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute_static: null plan");
+    plan->last_launches = 0;
+    if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute_static: call grid_plan_set_samples first");
+    if (plan->n_vis == 0) return GRID_OK;                              // R23
+    if (!uvw || !vis || !weights || !conv_kernel || !grid)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_static: null array argument");
+    if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
+        return fail(GRID_ERR_INVALID_ARG, "grid_execute_static: array arguments must be 16-byte aligned");
+    const size_t need = grid_plan_workspace_bytes(plan);
+    if (need > (size_t)GRID_STATIC_SCRATCH_BYTES)
+        return fail(GRID_ERR_UNSUPPORTED, "grid_execute_static: %lld samples need %zu bytes of workspace, the static scratch array "
+                    "holds %u (about 1.2 million samples per call): grid the input in several calls, or use grid_execute "
+                    "with grid_plan_set_workspace", plan->n_vis, need, (unsigned)GRID_STATIC_SCRATCH_BYTES);
+    void* scratch = nullptr;
+    const int rc0 = static_scratch_pointer(&scratch);
+    if (rc0 != GRID_OK) return rc0;
+    grid_plan call = *plan;                          // the caller's plan keeps its own workspace, if it has one
+    call.workspace = scratch;
+    call.workspace_bytes = GRID_STATIC_SCRATCH_BYTES;
+    // execute_impl clears the head of the workspace (queue counter, hop statistics, chunk-order bins) on `stream`
+    // before the first kernel; records, chunk order and tap table are fully rewritten before they are read.
+    const int rc = execute_impl(&call, uvw, nullptr, plan->n_vis, vis, weights, conv_kernel, grid, (cudaStream_t)stream);
+    plan->last_launches = call.last_launches;
+    return rc;
+}
+
 int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const float* weights, void* out_records,
                   float* out_vis, long long* out_count, grid_stream_t stream_) {
     cudaStream_t stream = (cudaStream_t)stream_;

@@ -186,6 +186,21 @@ int grid_plan_set_traversal(grid_plan* plan, int mode, int time_block);
  * the L2 (default).  Variant 3 only; ignored otherwise. */
 int grid_plan_set_chunk_order(grid_plan* plan, int mode);
 
+/* Order in which grid_execute hands the samples to the gridding kernel (the result is the same sum in a different
+ * order, pin P11; the gain of register accumulation depends on "the coordinates and ordering of the
+ * data": an accumulator is flushed when its cell changes):
+ *   1 = cell order: the a1 pass sorts the samples by the grid cell of their footprint origin (counting sort: per-cell
+ *       histogram, prefix sum, scatter of 16-byte records that carry the sample's index, or for one polarisation the
+ *       pre-weighted visibility; 5 launches instead of 1).  Consecutive samples then mostly share their cell and
+ *       flushes become rare.  Needs the warp kernel (variant 3) and 4 bytes per grid cell + 4 bytes per sample more
+ *       workspace: call grid_plan_workspace_bytes / grid_plan_set_workspace AFTER this call.  The layout hint, the
+ *       traversal mode and the chunk order are then irrelevant.
+ *   0 = input order (chunks of the caller's baseline-major order, walked as grid_plan_set_traversal says).
+ *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, else input order.
+ * grid_execute only: grid_execute_static, grid_execute_compressed (its input is already ordered by the caller),
+ * grid_execute_dense* and grid_degrid always use input order. */
+int grid_plan_set_sample_order(grid_plan* plan, int mode);
+
 /* Variant 3, n_pol = 4: spread the polarisations of one grid point over `lanes` adjacent threads
  * (1 or 2).  With 2, the two 16-byte atomics of a 32-byte grid point leave in one instruction and
  * cost the L2 one sector operation instead of two.  Set the block (cu, cv) first; returns
@@ -214,7 +229,7 @@ int grid_plan_autotune(grid_plan* plan, long long n_samples, unsigned int seed, 
 
 /* HOST out[20]: variant, cu, cv, bin_u, bin_v, team_threads, teams_per_cta, threads_per_cta, batch,
  * chunk, ctas_per_sm, smem_bytes, n_sm, traversal mode, time_block, chunk order mode,
- * polarisation split, warp groups per CTA, taps in global memory (0/1), 0. */
+ * polarisation split, warp groups per CTA, taps in global memory (0/1), sample order in effect (1 = cell order). */
 int grid_plan_get_info(const grid_plan* plan, int* out);
 
 /* Measurement hook: two caller-owned cudaEvent_t (passed as void*) that the following grid_execute

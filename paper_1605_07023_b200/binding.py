@@ -17,7 +17,7 @@ GRID_OK, GRID_ERR_INVALID_ARG, GRID_ERR_UNSUPPORTED, GRID_ERR_CUDA, GRID_ERR_STA
 EXPORTS = (
     "grid_plan_create", "grid_plan_set_samples", "grid_plan_set_layout", "grid_plan_workspace_bytes",
     "grid_plan_set_workspace", "grid_execute", "grid_execute_static", "grid_compress", "grid_execute_compressed", "grid_execute_dense", "grid_execute_dense_pol", "grid_degrid", "grid_plan_set_degrid_gather", "grid_quantise", "grid_plan_set_tuning",
-    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_debug_counters", "grid_plan_destroy", "grid_last_error",
+    "grid_plan_get_info", "grid_plan_set_traversal", "grid_plan_set_kernel_events", "grid_plan_set_chunk_order", "grid_plan_set_sample_order", "grid_plan_set_pol_split", "grid_plan_autotune", "grid_plan_autotune_candidates", "grid_plan_last_launches", "grid_plan_debug_counters", "grid_plan_destroy", "grid_last_error",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -48,6 +48,7 @@ _lib.grid_plan_get_info.argtypes = [_vp, _vp]
 _lib.grid_plan_set_traversal.argtypes = [_vp, _int, _int]
 _lib.grid_plan_set_kernel_events.argtypes = [_vp, _vp, _vp]
 _lib.grid_plan_set_chunk_order.argtypes = [_vp, _int]
+_lib.grid_plan_set_sample_order.argtypes = [_vp, _int]
 _lib.grid_plan_set_pol_split.argtypes = [_vp, _int]
 _lib.grid_plan_autotune_candidates.argtypes = [_vp, _vp, _int]
 _lib.grid_plan_autotune.argtypes = [_vp, _ll, ctypes.c_uint, _vp, _int, _vp]
@@ -90,7 +91,7 @@ def _stream(stream):
 
 
 INFO_FIELDS = ("variant", "cu", "cv", "bin_u", "bin_v", "team_threads", "teams_per_cta",
-               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block", "chunk_order", "pol_split", "groups_per_cta", "taps_global")
+               "threads_per_cta", "batch", "chunk", "ctas_per_sm", "smem_bytes", "n_sm", "traversal", "time_block", "chunk_order", "pol_split", "groups_per_cta", "taps_global", "sample_order")
 
 
 class GridPlan:
@@ -145,6 +146,9 @@ class GridPlan:
 
     def set_chunk_order(self, mode=-1):
         _check(_lib.grid_plan_set_chunk_order(self._h, mode), "grid_plan_set_chunk_order")
+
+    def set_sample_order(self, mode=-1):
+        _check(_lib.grid_plan_set_sample_order(self._h, mode), "grid_plan_set_sample_order")
 
     def autotune_candidates(self):
         """grid_plan_autotune_candidates: list of (cu, cv, pol_split) blocks that fit this plan, the current one first."""
@@ -328,6 +332,8 @@ def grid_visibilities(grid_size, support, oversample, n_wplanes, n_pol, uvw, vis
                 plan.set_traversal(tuning.pop("traversal", -1), tuning.pop("time_block", 0))
             if "chunk_order" in tuning:
                 plan.set_chunk_order(tuning.pop("chunk_order"))
+            if "sample_order" in tuning:
+                plan.set_sample_order(tuning.pop("sample_order"))
             if "pol_split" in tuning:          # before the block: (cu, cv) is validated against it
                 plan.set_pol_split(tuning.pop("pol_split"))
             if tuning:

@@ -435,6 +435,19 @@ grid_warp_kernel(const GridParams gp) {
             if (k >= count_of(cg, b)) continue;
             const uint32_t g = sample_of(cg, (b << bshift) + k);
             if (!GRIDB200_CHK(g < n_vis32, kChkSampleIndex) || !GRIDB200_CHK(kk < slots && st < 2, kChkRawSlot)) continue;
+            if (gp.sorted) {
+                // cell order: the record carries the index of its visibilities (P > 1) or the pre-weighted
+                // visibility itself (P = 1)
+                const uint4* src = reinterpret_cast<const uint4*>(gp.recs) + g;
+                cp_async_16(rrec + kk, src);
+                if constexpr (!DEGRID && P > 1) {
+                    const uint32_t vi = __ldg(reinterpret_cast<const uint32_t*>(src) + 3);
+                    if (!GRIDB200_CHK(vi < n_vis32, kChkSampleIndex)) continue;
+#pragma unroll
+                    for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + (size_t)vi * P + q);
+                }
+                continue;
+            }
             if (gp.rec16) {
                 cp_async_16(rrec + kk, reinterpret_cast<const uint4*>(gp.recs) + g);
             } else {
@@ -513,7 +526,10 @@ grid_warp_kernel(const GridParams gp) {
                 cvis[(size_t)ck * P] = make_float2(w, __uint_as_float(code));
             } else if constexpr (P == 1) {
                 float2 v = make_float2(0.f, 0.f);
-                if (valid) { v = rvis[kk]; v.x *= w; v.y *= w; }        // skipped: exact zeros, whatever the input holds
+                if (valid) {                                            // skipped: exact zeros, whatever the input holds
+                    if (gp.sorted) { const uint4 rec = rrec[kk]; v = make_float2(__uint_as_float(rec.z), __uint_as_float(rec.w)); }
+                    else { v = rvis[kk]; v.x *= w; v.y *= w; }
+                }
                 cvis[ck] = v;
             } else {
                 // pre-weighting, 16 bytes at a time

@@ -13,6 +13,7 @@
 #include "compress.cuh"
 #include "degrid_kernel.cuh"
 #include "quantise.cuh"
+#include "cell_sort.cuh"
 
 using namespace gridb200;
 
@@ -50,6 +51,7 @@ struct grid_plan {
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
     int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on
+    int sample_order;                     // grid_plan_set_sample_order: -1 auto, 0 input order, 1 sorted by grid cell
     int n_sm, max_smem;
     int last_launches;
     int user_tuned;                       // set_tuning / set_pol_split was called: set_samples keeps the block
@@ -268,6 +270,31 @@ size_t tap_table_bytes(const grid_plan* p) {
     return p->taps_global ? (size_t)tap_rows(p) * 2 * p->Sk * sizeof(float2) : 0;
 }
 
+// Cell order (cell_sort.cuh): grid_execute sorts the samples by grid cell in its a1 pass.  Automatic when the
+// input is large enough for the extra launches to pay and the per-cell histogram is not much larger than the
+// input itself (a sparse input on a huge grid would spend its time scanning empty cells).
+constexpr long long kCellSortMinSamples = 1 << 20;
+bool cell_sort_possible(const grid_plan* p) {
+    return p->variant == 3 && !p->dense && p->n_vis > 0 && p->n_vis < 0x7fffffffLL;
+}
+bool cell_sort_on(const grid_plan* p) {
+    if (p->sample_order == 0 || !cell_sort_possible(p)) return false;
+    if (p->sample_order > 0) return true;
+    return p->n_vis >= kCellSortMinSamples && (long long)p->N * p->N <= 8 * p->n_vis;
+}
+size_t cell_hist_entries(const grid_plan* p) {
+    return ((size_t)p->N * p->N + 1 + kScanTile - 1) / kScanTile * kScanTile;
+}
+// [histogram / offsets][block sums][ranks]
+size_t cell_sums_offset(const grid_plan* p) { return cell_hist_entries(p) * sizeof(uint32_t); }
+size_t cell_ranks_offset(const grid_plan* p) {
+    return cell_sums_offset(p) + ((cell_hist_entries(p) / kScanTile * sizeof(uint32_t) + 255) & ~(size_t)255);
+}
+size_t cell_sort_bytes(const grid_plan* p) {
+    return cell_sort_on(p) ? cell_ranks_offset(p) + (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(uint32_t) : 0;
+}
+size_t cell_sort_offset(const grid_plan* p) { return (tap_table_offset(p) + tap_table_bytes(p) + 255) & ~(size_t)255; }
+
 // Derive bins, team shape and shared-memory footprint from the tuning; validate.
 int derive(grid_plan* p) {
     if (p->variant == 0) {
@@ -380,6 +407,7 @@ void default_tuning(grid_plan* p) {
     p->ctas_per_sm = 2;
     p->traversal = -1;
     p->sort_chunks = -1;
+    p->sample_order = -1;
     p->pol_split = 1;
     p->time_block = 64;
     // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
@@ -571,6 +599,7 @@ int grid_plan_set_samples(grid_plan* plan, long long n_vis) {
         default_tuning(&trial);
         trial.traversal = plan->traversal; trial.time_block = plan->time_block;     // set by their own calls
         trial.sort_chunks = plan->sort_chunks;
+        trial.sample_order = plan->sample_order;
         if (derive(&trial) == GRID_OK) *plan = trial;
         g_err[0] = 0;
     }
@@ -586,7 +615,7 @@ int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_ch
 
 size_t grid_plan_workspace_bytes(const grid_plan* plan) {
     if (!plan || plan->n_vis < 0) return 0;
-    return tap_table_offset(plan) + tap_table_bytes(plan);
+    return cell_sort_on(plan) ? cell_sort_offset(plan) + cell_sort_bytes(plan) : tap_table_offset(plan) + tap_table_bytes(plan);
 }
 
 int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
@@ -740,7 +769,7 @@ int grid_plan_get_info(const grid_plan* plan, int* out) {
     const int v[20] = {plan->variant, plan->cu, plan->cv, plan->bin_u, plan->bin_v, plan->team_threads,
                        plan->teams_per_cta, plan->threads, plan->batch, plan->chunk, plan->ctas_per_sm,
                        plan->smem_bytes, plan->n_sm, plan->traversal, plan->time_block, plan->sort_chunks,
-                       plan->pol_split, plan->groups_per_cta, plan->taps_global, 0};
+                       plan->pol_split, plan->groups_per_cta, plan->taps_global, cell_sort_on(plan) ? 1 : 0};
     memcpy(out, v, sizeof(v));
     return GRID_OK;
 }
@@ -776,6 +805,14 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode) {
     if (!plan || mode < -1 || mode > 1)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_chunk_order: mode in {-1,0,1}");
     plan->sort_chunks = mode;
+    return GRID_OK;
+}
+
+int grid_plan_set_sample_order(grid_plan* plan, int mode) {
+    if (!plan || mode < -1 || mode > 1) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_sample_order: mode must be -1, 0 or 1");
+    if (mode == 1 && plan->variant != 3)
+        return fail(GRID_ERR_UNSUPPORTED, "grid_plan_set_sample_order: cell order needs the warp kernel (variant 3)");
+    plan->sample_order = mode;
     return GRID_OK;
 }
 
@@ -824,8 +861,10 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     uint32_t* bins = counters + 64;
     uint32_t* order = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes + records_bytes(plan));
 
+    // cell order: the a1 pass sorts the samples by grid cell (cell_sort.cuh); chunks are runs of the sorted records
+    const bool sorted = !ext_recs && !degrid_out && n_vis == plan->n_vis && cell_sort_on(plan);
     // the layout hint is used only if it is consistent with the sample count
-    const bool have_layout = !ext_recs && plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
+    const bool have_layout = !sorted && !ext_recs && plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
                              (long long)plan->n_baselines * plan->n_times * plan->n_channels == n_vis;
     const int n_chan = have_layout ? plan->n_channels : 0, n_times = have_layout ? plan->n_times : 0;
     float* hop_stats = reinterpret_cast<float*>(counters + 2);
@@ -835,7 +874,29 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     // reset the chunk queue and the hop statistics, then a1: quantise pass
     if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
-    if (!ext_recs) {
+    if (sorted) {
+        unsigned char* scratch = reinterpret_cast<unsigned char*>(plan->workspace) + cell_sort_offset(plan);
+        uint32_t* hist = reinterpret_cast<uint32_t*>(scratch);
+        uint32_t* sums = reinterpret_cast<uint32_t*>(scratch + cell_sums_offset(plan));
+        uint32_t* ranks = reinterpret_cast<uint32_t*>(scratch + cell_ranks_offset(plan));
+        const size_t entries = cell_hist_entries(plan);
+        const unsigned scan_blocks = (unsigned)(entries / kScanTile);
+        if (cudaMemsetAsync(hist, 0, entries * sizeof(uint32_t), stream) != cudaSuccess)
+            return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
+        const unsigned blocks = (unsigned)(((n_vis + 3) / 4 + 255) / 256);
+        const QuantParams qp = quant_params(plan);
+        cell_count_kernel<<<blocks, 256, 0, stream>>>(uvw, n_vis, qp, hist, ranks);
+        cell_scan_reduce_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
+        cell_scan_sums_kernel<<<1, 1024, 0, stream>>>(sums, (int)scan_blocks);
+        cell_scan_apply_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
+        if (plan->P == 1)
+            cell_scatter_kernel<true><<<blocks, 256, 0, stream>>>(uvw, weights, reinterpret_cast<const float2*>(vis), n_vis, qp,
+                                                                  hist, ranks, reinterpret_cast<uint4*>(recs));
+        else
+            cell_scatter_kernel<false><<<blocks, 256, 0, stream>>>(uvw, weights, nullptr, n_vis, qp, hist, ranks,
+                                                                   reinterpret_cast<uint4*>(recs));
+        plan->last_launches += 5;
+    } else if (!ext_recs) {
         const long long threads = (n_vis + 3) / 4;
         const long long blocks = (threads + 255) / 256;
         quantise_kernel<<<(unsigned)blocks, 256, 0, stream>>>(uvw, recs, n_vis, quant_params(plan), hop_stats,
@@ -853,6 +914,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.vis_out = reinterpret_cast<float2*>(degrid_out);
     gp.counters = counters;
     gp.rec16 = (plan->variant == 3 && !ext_recs) ? 1 : 0;
+    gp.sorted = sorted ? 1 : 0;
     gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->variant == 3 ? plan->Sk : plan->S;
     gp.n_rows = plan->variant == 3 ? tap_rows(plan) : plan->W * plan->O;
@@ -949,7 +1011,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
             const long long chunks_a = (n_vis + gp.chunk - 1) / gp.chunk;
             const long long max_chunks = chunks_a > gp.n_chunks_b ? chunks_a : gp.n_chunks_b;
             const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
-            const bool want = plan->sort_chunks > 0 || (plan->sort_chunks < 0 && grid_bytes > ((size_t)256 << 20));
+            const bool want = !sorted && (plan->sort_chunks > 0 || (plan->sort_chunks < 0 && grid_bytes > ((size_t)256 << 20)));
             const bool worth = plan->sort_chunks > 0 || max_chunks >= 4LL * ctas_hint(plan);   // auto: only when chunks queue up
             if (want && worth && max_chunks <= (long long)order_capacity(plan)) {
                 int ts = 0;
@@ -1029,7 +1091,9 @@ int grid_execute_static(grid_plan* plan, const float* uvw, const float* vis, con
         return fail(GRID_ERR_INVALID_ARG, "grid_execute_static: null array argument");
     if ((((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)conv_kernel | (uintptr_t)grid) & 15) != 0)
         return fail(GRID_ERR_INVALID_ARG, "grid_execute_static: array arguments must be 16-byte aligned");
-    const size_t need = grid_plan_workspace_bytes(plan);
+    grid_plan call = *plan;                          // the caller's plan keeps its own workspace, if it has one
+    call.sample_order = 0;                           // input order: the sort's histogram of the grid would not fit
+    const size_t need = grid_plan_workspace_bytes(&call);
     if (need > (size_t)GRID_STATIC_SCRATCH_BYTES)
         return fail(GRID_ERR_UNSUPPORTED, "grid_execute_static: %lld samples need %zu bytes of workspace, the static scratch array "
                     "holds %u (about 1.2 million samples per call): grid the input in several calls, or use grid_execute "
@@ -1037,7 +1101,6 @@ int grid_execute_static(grid_plan* plan, const float* uvw, const float* vis, con
     void* scratch = nullptr;
     const int rc0 = static_scratch_pointer(&scratch);
     if (rc0 != GRID_OK) return rc0;
-    grid_plan call = *plan;                          // the caller's plan keeps its own workspace, if it has one
     call.workspace = scratch;
     call.workspace_bytes = GRID_STATIC_SCRATCH_BYTES;
     // execute_impl clears the head of the workspace (queue counter, hop statistics, chunk-order bins) on `stream`

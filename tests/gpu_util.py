@@ -22,6 +22,8 @@ def run_gpu(N, S, O, W, P, uvw, vis, weights, kernel, layout=None, tuning=None, 
                 plan.set_traversal(tuning.pop("traversal", -1), tuning.pop("time_block", 0))
             if "chunk_order" in tuning:
                 plan.set_chunk_order(tuning.pop("chunk_order"))
+            if "sample_order" in tuning:
+                plan.set_sample_order(tuning.pop("sample_order"))
             if "pol_split" in tuning:          # before the block: (cu, cv) is validated against it
                 plan.set_pol_split(tuning.pop("pol_split"))
             if tuning:

@@ -1,0 +1,121 @@
+"""-m gpu: grid_execute with the samples sorted by grid cell in the a1 pass (grid_plan_set_sample_order,
+csrc/cell_sort.cuh) against the float64 oracle on the same seeded inputs, through the C ABI.  The sum is
+order-independent (pin P11), so the tolerances are the ones of every other gridding test (R20)."""
+import numpy as np
+import pytest
+
+from paper_1605_07023_b200 import synth
+from gpu_util import assert_parity, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+# every instantiated block of the warp kernel
+WARP = [(2, 2, 1), (4, 2, 1), (4, 4, 1), (8, 4, 1), (2, 2, 2), (4, 2, 2), (4, 4, 2), (2, 2, 4), (4, 2, 4)]
+
+
+@pytest.mark.parametrize("cu,cv,P", WARP)
+@pytest.mark.parametrize("S", [4, 8, 16, 32])
+def test_cell_order_every_warp_block(oracle_mod, cu, cv, P, S):
+    # ragged tail (n not a multiple of 4, batch or chunk), samples off the grid and with non-finite coordinates
+    # (they sort behind all others and must contribute exact zeros), jumps larger than the support, 3 planes
+    if cu > S or cv > S:
+        pytest.skip("block larger than the support")
+    N, O, W, n = 128, 4, 3, 20_003
+    uvw, vis, wts, kernel = synth.random_problem(7000 + 100 * cu + 10 * cv + P + S, n, N, S, O, W, P,
+                                                 spread=0.5, walk=1.5)
+    uvw[7000:7010, 0] = np.nan
+    vis[7000:7010] = np.inf
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    for batch, chunk in ((32, 300), (8, 64)):
+        got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                            tuning=dict(sample_order=1, variant=3, cu=cu, cv=cv, threads_per_cta=1024, batch=batch, chunk=chunk))
+        assert (info["variant"], info["cu"], info["cv"], info["sample_order"]) == (3, cu, cv, 1)
+        assert info["launches"] == 6, info                       # count, three scan kernels, scatter, gridding
+        assert_parity(got, ref, f"cell order C={cu}x{cv} P={P} S={S} batch={batch} {info}")
+
+
+@pytest.mark.parametrize("cu,cv", [(2, 2), (4, 2), (4, 4)])
+@pytest.mark.parametrize("S", [8, 16])
+def test_cell_order_pol_split(oracle_mod, cu, cv, S):
+    N, O, W, P, n = 160, 8, 2, 4, 15_001
+    uvw, vis, wts, kernel = synth.random_problem(7500 + 10 * cu + cv + S, n, N, S, O, W, P, spread=0.45, walk=0.8)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel,
+                        tuning=dict(sample_order=1, variant=3, cu=cu, cv=cv, pol_split=2))
+    assert (info["pol_split"], info["sample_order"]) == (2, 1)
+    assert_parity(got, ref, f"cell order C={cu}x{cv} PS=2 S={S}")
+
+
+@pytest.mark.parametrize("S,P,N", [(7, 1, 512), (12, 4, 200), (13, 2, 97), (3, 1, 64), (40, 1, 300), (64, 4, 256),
+                                   (100, 1, 512), (128, 1, 512)])
+def test_cell_order_padded_and_large_supports(oracle_mod, S, P, N):
+    # supports that are not powers of two (zero-padded taps: the key is the cell of the PADDED footprint's origin),
+    # 64-bit masks (S = 64) and tiled bins (S = 128: four queue entries per chunk)
+    O, W, n = 4, 2, 6_007
+    uvw, vis, wts, kernel = synth.random_problem(7700 + S + P, n, N, S, O, W, P, spread=0.5, walk=2.0)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(sample_order=1))
+    assert (info["variant"], info["sample_order"]) == (3, 1), info
+    assert_parity(got, ref, f"cell order S={S} P={P} N={N} {info}")
+
+
+def test_cell_order_degenerate_inputs(oracle_mod):
+    N, S, O, W, P = 64, 8, 8, 1, 4
+    rng = np.random.default_rng(5)
+    kernel = (rng.normal(size=(W, O, S)) + 1j * rng.normal(size=(W, O, S))).astype(np.complex64)
+    # (a) every sample in ONE cell (one histogram bin takes all the atomics; every chunk flushes once)
+    n = 50_001
+    uvw = np.zeros((n, 3), np.float32)
+    uvw[:, :2] = rng.uniform(0.0, 0.99, (n, 2)) + 3.0
+    vis = (rng.normal(size=(n, P)) + 1j * rng.normal(size=(n, P))).astype(np.complex64)
+    wts = rng.uniform(0.5, 1.0, n).astype(np.float32)
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, _ = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(sample_order=1))
+    assert_parity(got, ref, "one cell")
+    # (b) every sample off the grid: the grid must stay exactly as it was
+    uvw_off = uvw + 1000.0
+    init = (rng.normal(size=(N, N, P)) + 1j * rng.normal(size=(N, N, P))).astype(np.complex64)
+    got, _ = run_gpu(N, S, O, W, P, uvw_off, vis, wts, kernel, tuning=dict(sample_order=1), grid_init=init)
+    assert np.array_equal(got, init)
+    # (c) one sample; (d) grid accumulated into (R10)
+    got, _ = run_gpu(N, S, O, W, P, uvw[:1], vis[:1], wts[:1], kernel, tuning=dict(sample_order=1), grid_init=init)
+    ref1 = oracle_mod.grid(N, S, O, W, P, uvw[:1], vis[:1], wts[:1], kernel) + init
+    assert_parity(got, ref1, "one sample onto a non-zero grid")
+
+
+def test_cell_order_edges_and_corners(oracle_mod):
+    # odd grid size whose N*N + 1 histogram entries are not a multiple of the scan tile, footprints in all four
+    # corners (first and last histogram bins), one polarisation (records carry the pre-weighted visibility)
+    N, S, O, W, P = 1001, 8, 8, 1, 1
+    rng = np.random.default_rng(11)
+    n = 40_003
+    uvw = np.zeros((n, 3), np.float32)
+    lo, hi = -(N // 2) + S / 2 - 1, (N - 1 - N // 2) - S / 2
+    uvw[:, 0] = rng.choice([lo + 0.3, hi + 0.4, 0.0], n) + rng.uniform(-0.2, 0.2, n)
+    uvw[:, 1] = rng.choice([lo + 0.3, hi + 0.4, 0.0], n) + rng.uniform(-0.2, 0.2, n)
+    vis = (rng.normal(size=(n, P)) + 1j * rng.normal(size=(n, P))).astype(np.complex64)
+    wts = rng.uniform(0.5, 1.0, n).astype(np.float32)
+    kernel = (rng.normal(size=(W, O, S)) + 1j * rng.normal(size=(W, O, S))).astype(np.complex64)
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    assert q["valid"].all() and q["i0"].min() == 0 and q["j0"].min() == 0 and q["i0"].max() == N - S and q["j0"].max() == N - S
+    ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+    got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(sample_order=1))
+    assert info["sample_order"] == 1
+    assert_parity(got, ref, "corners")
+
+
+def test_cell_order_is_the_default_for_large_inputs(oracle_mod):
+    # automatic mode: 2^20 samples or more on a grid of at most 8 n_vis cells; same answer as input order
+    cfg = synth.shrink(synth.get_config("cfg1"), n_ant=24, n_times=64, n_chan=64, grid_size=1024)
+    wl = synth.make_workload(cfg)
+    assert cfg.n_vis >= 1 << 20
+    args = (cfg.grid_size, cfg.support, cfg.oversample, cfg.n_wplanes, cfg.n_pol, wl.uvw, wl.vis, wl.weights, wl.kernel)
+    layout = (cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    got, info = run_gpu(*args, layout=layout)
+    assert info["sample_order"] == 1 and info["launches"] == 6, info
+    got0, info0 = run_gpu(*args, layout=layout, tuning=dict(sample_order=0))
+    assert info0["sample_order"] == 0 and info0["launches"] == 2, info0
+    lo = cfg.grid_size // 2 + 40
+    ref = oracle_mod.grid(*args, rows=(lo, lo + 8))
+    assert_parity(got[lo:lo + 8], ref, "cell order, row band")
+    assert_parity(got0[lo:lo + 8], ref, "input order, row band")

@@ -407,7 +407,6 @@ void default_tuning(grid_plan* p) {
     p->ctas_per_sm = 2;
     p->traversal = -1;
     p->sort_chunks = -1;
-    p->sample_order = -1;
     p->pol_split = 1;
     p->time_block = 64;
     // first guess per (S, P); refined by the autotune sweep -- see DESIGN.md
@@ -450,6 +449,21 @@ void default_tuning(grid_plan* p) {
         // bound by the latency of a team's sequential walk, not by issue slots: small blocks spread a bin over more
         // threads (cfg0: 2x2 runs in 0.025 ms where 4x4 needs 0.054 ms).
         if (trial.n_vis >= 0 && trial.n_vis < 4096LL * trial.n_sm && logs <= 4) { trial.cu = 2; trial.cv = 2; }
+        // Cell order (cell_sort.cuh): flushes are rare, so the block is chosen for the multiply-add loop alone and
+        // lane pairing no longer pays (sweep of every instantiated block on the 11 large BASELINE.json workloads,
+        // profiles/r2_cell_order.md); short chunks keep the CTAs in flight on neighbouring cells.
+        if (cell_sort_on(&trial) && logs <= 5 && trial.P != 2) {
+            trial.pol_split = 1;
+            if (trial.P >= 4) {
+                if (logs <= 3) { trial.cu = 2; trial.cv = 2; trial.pol_split = logs == 2 ? 2 : 1; }
+                else { trial.cu = 4; trial.cv = 2; }
+            } else {
+                if (logs == 2) { trial.cu = 2; trial.cv = 2; }
+                else if (logs == 3) { trial.cu = 4; trial.cv = 2; }
+                else { trial.cu = 8; trial.cv = 4; }
+            }
+            if (logs <= 4) trial.chunk = 128;
+        }
         // several teams share a warp at small supports: shrink the batch until all warps fit
         while (trial.batch > 8) {
             grid_plan probe = trial;
@@ -582,6 +596,7 @@ grid_plan* grid_plan_create(int grid_size, int support, int oversample, int n_wp
     p->N = grid_size; p->S = support; p->O = oversample; p->W = n_wplanes; p->P = n_pol;
     p->Sk = padded_support(support, grid_size, n_wplanes, oversample);
     p->n_vis = -1;
+    p->sample_order = -1;
     p->n_sm = n_sm;
     p->max_smem = max_smem - 1024;      // leave room for static shared memory
     default_tuning(p);
@@ -591,18 +606,21 @@ grid_plan* grid_plan_create(int grid_size, int support, int oversample, int n_wp
 
 void grid_plan_destroy(grid_plan* plan) { delete plan; }
 
+// the default block depends on the size of the input and on the order the samples are gridded in
+static void retune(grid_plan* plan) {
+    if (plan->user_tuned) return;
+    grid_plan trial = *plan;
+    default_tuning(&trial);
+    trial.traversal = plan->traversal; trial.time_block = plan->time_block;     // set by their own calls
+    trial.sort_chunks = plan->sort_chunks;
+    if (derive(&trial) == GRID_OK) *plan = trial;
+    g_err[0] = 0;
+}
+
 int grid_plan_set_samples(grid_plan* plan, long long n_vis) {
     if (!plan || n_vis < 0) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_samples: invalid argument");
     plan->n_vis = n_vis;
-    if (!plan->user_tuned) {                         // the default block depends on the size of the input
-        grid_plan trial = *plan;
-        default_tuning(&trial);
-        trial.traversal = plan->traversal; trial.time_block = plan->time_block;     // set by their own calls
-        trial.sort_chunks = plan->sort_chunks;
-        trial.sample_order = plan->sample_order;
-        if (derive(&trial) == GRID_OK) *plan = trial;
-        g_err[0] = 0;
-    }
+    retune(plan);
     return GRID_OK;
 }
 
@@ -813,6 +831,7 @@ int grid_plan_set_sample_order(grid_plan* plan, int mode) {
     if (mode == 1 && plan->variant != 3)
         return fail(GRID_ERR_UNSUPPORTED, "grid_plan_set_sample_order: cell order needs the warp kernel (variant 3)");
     plan->sample_order = mode;
+    retune(plan);
     return GRID_OK;
 }
 

@@ -45,6 +45,9 @@ def parse_args():
                     help="compress once outside the timed region (PAPER.md:69, 113) and time grid_execute_compressed; "
                          "the rate then counts compressed samples, as the paper's does")
     ap.add_argument("--tuning", default="", help="e.g. cu=2,cv=2,threads_per_cta=256")
+    ap.add_argument("--sample-order", type=int, default=-1, choices=[-1, 0, 1],
+                    help="grid_plan_set_sample_order: 1 = the a1 pass sorts the samples by grid cell, 0 = input "
+                         "(baseline-major) order, -1 = the library's choice (default)")
     ap.add_argument("--no-per-config", action="store_true",
                     help="skip the per_config table (every BASELINE.json config, device-resident, with an oracle row band)")
     ap.add_argument("--per-config-steps", type=int, default=5)
@@ -236,7 +239,7 @@ def reduce_over_ranks(times_ms, units, device, world):
 ALL_CONFIGS = ["cfg0", "cfg1", "cfg2", "cfg3"] + [f"cfg4_S{s}_P{p}" for s in (4, 8, 16, 32) for p in (1, 4)]
 
 
-def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False):
+def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False, sample_order=-1):
     """One BASELINE.json config, device-resident: K timed grid_execute calls (CUDA events on the launching
     stream, L2 scrubbed between steps when the inputs could stay in it), the hot kernel's own time, and the
     rel-L2 / max-abs error of one band of grid rows against the float64 oracle (row-restricted mode)."""
@@ -250,6 +253,7 @@ def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False):
     plan = binding.GridPlan(N, S, O, W, P)
     plan.set_samples(cfg.n_vis)
     plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    plan.set_sample_order(sample_order)
     tuned = None
     if autotune:                                               # time every candidate block, keep the fastest
         default = plan.info()
@@ -306,6 +310,7 @@ def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False):
                          "kernel_ms": kernel_ms, "kernel": kernel_template_name(info, P, S, "grid", N)},
             "block": "%dx%d, pol split %d, %d threads, batch %d" % (info["cu"], info["cv"], info["pol_split"],
                                                                     info["threads_per_cta"], info["batch"]),
+            "sample_order": "cell" if info["sample_order"] else "input", "a1_pass_ms": ms - kernel_ms,
             "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err, "autotune": tuned}
 
 
@@ -443,6 +448,7 @@ def run_ours(args):
     plan = binding.GridPlan(N, S, O, W, P)
     plan.set_samples(cfg.n_vis)
     plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+    plan.set_sample_order(args.sample_order)
     tuning = parse_tuning(args.tuning)
     if tuning:
         plan.set_tuning(**tuning)
@@ -625,7 +631,8 @@ def run_ours(args):
             plan.destroy()
             del d_uvw, d_vis, d_wts, grid, h_uvw, h_vis, h_wts
             torch.cuda.empty_cache()
-            line["per_config"] = [measure_config(n, args.per_config_steps, 3, dev, autotune=args.autotune) for n in ALL_CONFIGS]
+            line["per_config"] = [measure_config(n, args.per_config_steps, 3, dev, autotune=args.autotune, sample_order=args.sample_order)
+                                  for n in ALL_CONFIGS]
         print(json.dumps(line), flush=True)
     plan.destroy()
     if world > 1:

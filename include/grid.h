@@ -197,8 +197,9 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode);
  *       traversal mode and the chunk order are then irrelevant.
  *   0 = input order (chunks of the caller's baseline-major order, walked as grid_plan_set_traversal says).
  *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, else input order.
- * grid_execute only: grid_execute_static, grid_execute_compressed (its input is already ordered by the caller),
- * grid_execute_dense* and grid_degrid always use input order. */
+ * Applies to grid_execute and grid_degrid (whose results then go back to their samples' places through the index in
+ * the record); grid_execute_static, grid_execute_compressed (its input is already ordered by the caller) and
+ * grid_execute_dense* always use input order. */
 int grid_plan_set_sample_order(grid_plan* plan, int mode);
 
 /* Variant 3, n_pol = 4: spread the polarisations of one grid point over `lanes` adjacent threads

@@ -519,7 +519,7 @@ grid_warp_kernel(const GridParams gp) {
                 else { c.y = xo * 8u; c.z = yo * 8u; c.w = mx | (my << 16); }
                 valid = (rec.x & 0x8000u) == 0;
                 if (valid) w = unit_w ? 1.f : __uint_as_float(rec.z);
-                if constexpr (DEGRID) code = sample_of(cg, (b << bshift) + k) | (valid ? 0u : 0x80000000u);
+                if constexpr (DEGRID) code = (gp.sorted ? rec.w : sample_of(cg, (b << bshift) + k)) | (valid ? 0u : 0x80000000u);
             }
             crec[ck] = c;
             if constexpr (DEGRID) {

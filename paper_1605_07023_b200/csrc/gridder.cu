@@ -881,7 +881,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     uint32_t* order = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes + records_bytes(plan));
 
     // cell order: the a1 pass sorts the samples by grid cell (cell_sort.cuh); chunks are runs of the sorted records
-    const bool sorted = !ext_recs && !degrid_out && n_vis == plan->n_vis && cell_sort_on(plan);
+    const bool sorted = !ext_recs && n_vis == plan->n_vis && cell_sort_on(plan);
     // the layout hint is used only if it is consistent with the sample count
     const bool have_layout = !sorted && !ext_recs && plan->n_channels > 0 && plan->n_times > 0 && plan->n_baselines > 0 &&
                              (long long)plan->n_baselines * plan->n_times * plan->n_channels == n_vis;
@@ -908,7 +908,7 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         cell_scan_reduce_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
         cell_scan_sums_kernel<<<1, 1024, 0, stream>>>(sums, (int)scan_blocks);
         cell_scan_apply_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
-        if (plan->P == 1)
+        if (plan->P == 1 && !degrid_out)           // degridding needs the sample's index: where its result goes
             cell_scatter_kernel<true><<<blocks, 256, 0, stream>>>(uvw, weights, reinterpret_cast<const float2*>(vis), n_vis, qp,
                                                                   hist, ranks, reinterpret_cast<uint4*>(recs));
         else

@@ -119,3 +119,60 @@ def test_cell_order_is_the_default_for_large_inputs(oracle_mod):
     ref = oracle_mod.grid(*args, rows=(lo, lo + 8))
     assert_parity(got[lo:lo + 8], ref, "cell order, row band")
     assert_parity(got0[lo:lo + 8], ref, "input order, row band")
+
+
+def _gpu_degrid_cell_order(N, S, O, W, P, uvw, wts, kernel, grid, tuning=None):
+    import torch
+    from paper_1605_07023_b200 import binding
+    dev = torch.device("cuda:0")
+    plan = binding.GridPlan(N, S, O, W, P)
+    try:
+        plan.set_samples(uvw.shape[0])
+        plan.set_sample_order(1)
+        if tuning:
+            plan.set_tuning(**tuning)
+        plan.allocate_workspace(dev)
+        assert plan.info()["sample_order"] == 1
+        out = plan.degrid(torch.from_numpy(uvw).to(dev), torch.from_numpy(wts).to(dev),
+                          torch.from_numpy(kernel).to(dev), torch.from_numpy(grid.astype(np.complex64)).to(dev))
+        torch.cuda.synchronize()
+        launches = plan.last_launches()
+        return out.cpu().numpy(), launches
+    finally:
+        plan.destroy()
+
+
+@pytest.mark.parametrize("S,P,W", [(7, 1, 3), (8, 4, 3), (16, 1, 3), (16, 2, 3), (32, 4, 3), (12, 4, 3), (40, 1, 3),
+                                   (64, 4, 2), (128, 1, 2), (16, 1, 700)])
+def test_degrid_in_cell_order(oracle_mod, S, P, W):
+    # degridding walks the samples in cell order too: every result must come back to ITS sample's place (the index
+    # travels in the record), skipped samples get exact zeros; tolerances as in tests/test_gpu_degrid.py (DESIGN R20)
+    N, O, n = (192 if S <= 40 else 384), 4, 9_973
+    uvw, _, wts, kernel = synth.random_problem(8100 + S + P, n, N, S, O, W, P, spread=0.52)
+    uvw[100:110, 0] = np.nan
+    rng = np.random.default_rng(S)
+    grid = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+    ref = oracle_mod.degrid(N, S, O, W, P, uvw, wts, kernel, grid)
+    got, launches = _gpu_degrid_cell_order(N, S, O, W, P, uvw, wts, kernel, grid)
+    got = got.astype(np.complex128)
+    assert launches >= 6, launches                               # the sort's five kernels + the degridding kernel
+    q = oracle_mod.quantise(N, S, O, W, uvw)
+    assert (q["valid"] == 0).sum() > 10
+    assert not got[q["valid"] == 0].any()
+    scale = np.sqrt(np.mean(np.abs(ref[q["valid"] == 1]) ** 2))
+    assert np.abs(got - ref).max() <= 2e-5 * scale * max(1.0, S / 8)
+    assert np.linalg.norm(got - ref) <= 1e-5 * np.linalg.norm(ref)
+
+
+def test_adjoint_identity_in_cell_order(oracle_mod):
+    # <grid(V), G> = <V, degrid(G)> (pin P7) on the CUDA pair, both in cell order
+    N, S, O, W, P, n = 256, 8, 8, 2, 4, 40_001
+    uvw, vis, wts, kernel = synth.random_problem(8300, n, N, S, O, W, P, spread=0.45, walk=0.7)
+    rng = np.random.default_rng(3)
+    G = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+    gridded, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(sample_order=1))
+    assert info["sample_order"] == 1
+    degridded, _ = _gpu_degrid_cell_order(N, S, O, W, P, uvw, wts, kernel, G)
+    lhs = np.vdot(gridded.astype(np.complex128), G.astype(np.complex128))          # as in tests/test_gpu_degrid.py
+    rhs = np.vdot(vis.astype(np.complex128), degridded.astype(np.complex128))
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs)

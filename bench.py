@@ -301,6 +301,22 @@ def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False, s
     plan.set_kernel_events(None, None)
     ms = float(np.mean([a.elapsed_time(b) for a, b in s_ev]))
     kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
+    # Context, not the metric: the same steps when the caller declares uvw and weights unchanged between calls
+    # (grid_plan_set_sample_order(plan, 2); the paper's own setting: quantisation and ordering are
+    # an offline pre-process reused every major cycle) -- the sorted records are kept and a step is the kernel alone.
+    kept_ms = None
+    if info["sample_order"]:
+        plan.set_sample_order(2)
+        plan.allocate_workspace(dev)
+        for _ in range(2):
+            plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(steps):
+            plan.execute(d_uvw, d_vis, d_wts, d_kern, grid)
+        b.record(stream)
+        torch.cuda.synchronize()
+        kept_ms = a.elapsed_time(b) / steps
     plan.destroy()
     rate = updates / (ms * 1e-3)
     return {"workload": name, "support": S, "n_pol": P, "grid": N, "n_wplanes": W, "n_vis": cfg.n_vis,
@@ -311,6 +327,9 @@ def measure_config(name, steps, warmup, dev, oracle_band=True, autotune=False, s
             "block": "%dx%d, pol split %d, %d threads, batch %d" % (info["cu"], info["cv"], info["pol_split"],
                                                                     info["threads_per_cta"], info["batch"]),
             "sample_order": "cell" if info["sample_order"] else "input", "a1_pass_ms": ms - kernel_ms,
+            "order_kept": None if kept_ms is None else {
+                "ms_per_step": kept_ms, "pct_fp32_roofline": 100.0 * updates / (kept_ms * 1e-3) * FLOPS_PER_UPDATE / (PEAK_FP32_TFLOPS * 1e12),
+                "what": "grid_plan_set_sample_order(plan, 2): caller declares uvw and weights unchanged, sorted records reused"},
             "l2_flushed_between_steps": flush_l2, "gpu_launches": launches, "oracle_band": err, "autotune": tuned}
 
 

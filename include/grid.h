@@ -192,9 +192,17 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode);
  *   1 = cell order: the a1 pass sorts the samples by the grid cell of their footprint origin (counting sort: per-cell
  *       histogram, prefix sum, scatter of 16-byte records that carry the sample's index, or for one polarisation the
  *       pre-weighted visibility; 5 launches instead of 1).  Consecutive samples then mostly share their cell and
- *       flushes become rare.  Needs the warp kernel (variant 3) and 4 bytes per grid cell + 4 bytes per sample more
- *       workspace: call grid_plan_workspace_bytes / grid_plan_set_workspace AFTER this call.  The layout hint, the
- *       traversal mode and the chunk order are then irrelevant.
+ *       flushes become rare.  Needs the warp kernel (variant 3) and 4 bytes per grid cell + 20 bytes per sample
+ *       more workspace (a sorted record has a 32-byte sector to itself): call grid_plan_workspace_bytes /
+ *       grid_plan_set_workspace AFTER this call.  The layout hint, the traversal mode and the chunk order are then
+ *       irrelevant.
+ *   2 = cell order, kept: as 1, and the sorted records stay in the workspace -- the following grid_execute and
+ *       grid_degrid calls on this plan skip the sort.  THE CALLER GUARANTEES that they pass the same uvw and weights
+ *       (the paper's case: compression and quantisation are "done as a pre-process and reused for every major
+ *       cycle"; only the visibilities change).  Any grid_plan_set_* call that changes samples,
+ *       workspace, tuning or order, grid_compress and grid_execute_dense* drop the kept records; call
+ *       grid_plan_set_sample_order(plan, 2) again after changing uvw or weights in place.  The workspace must not be
+ *       shared with another plan meanwhile.
  *   0 = input order (chunks of the caller's baseline-major order, walked as grid_plan_set_traversal says).
  *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, else input order.
  * Applies to grid_execute and grid_degrid (whose results then go back to their samples' places through the index in

@@ -438,13 +438,18 @@ grid_warp_kernel(const GridParams gp) {
             if (gp.sorted) {
                 // cell order: the record carries the index of its visibilities (P > 1) or the pre-weighted
                 // visibility itself (P = 1)
-                const uint4* src = reinterpret_cast<const uint4*>(gp.recs) + g;
+                const uint4* src = reinterpret_cast<const uint4*>(gp.recs) + (size_t)g * gp.sorted_stride;
                 cp_async_16(rrec + kk, src);
-                if constexpr (!DEGRID && P > 1) {
-                    const uint32_t vi = __ldg(reinterpret_cast<const uint32_t*>(src) + 3);
-                    if (!GRIDB200_CHK(vi < n_vis32, kChkSampleIndex)) continue;
+                if constexpr (!DEGRID) {
+                    if (P > 1 || gp.sorted == 2) {
+                        const uint32_t vi = __ldg(reinterpret_cast<const uint32_t*>(src) + 3);
+                        if (!GRIDB200_CHK(vi < n_vis32, kChkSampleIndex)) continue;
+                        if constexpr (P == 1) cp_async_8(rvis + kk, gp.vis + vi);
+                        else {
 #pragma unroll
-                    for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + (size_t)vi * P + q);
+                            for (int q = 0; q < P; q += 2) cp_async_16(rvis + (size_t)kk * P + q, gp.vis + (size_t)vi * P + q);
+                        }
+                    }
                 }
                 continue;
             }
@@ -527,7 +532,7 @@ grid_warp_kernel(const GridParams gp) {
             } else if constexpr (P == 1) {
                 float2 v = make_float2(0.f, 0.f);
                 if (valid) {                                            // skipped: exact zeros, whatever the input holds
-                    if (gp.sorted) { const uint4 rec = rrec[kk]; v = make_float2(__uint_as_float(rec.z), __uint_as_float(rec.w)); }
+                    if (gp.sorted == 1) { const uint4 rec = rrec[kk]; v = make_float2(__uint_as_float(rec.z), __uint_as_float(rec.w)); }
                     else { v = rvis[kk]; v.x *= w; v.y *= w; }
                 }
                 cvis[ck] = v;

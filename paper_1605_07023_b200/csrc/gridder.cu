@@ -51,7 +51,8 @@ struct grid_plan {
     int degrid_gather;                    // 1: grid_degrid always uses the gather kernel (diagnostic)
     int pol_split;                        // variant 3: lanes sharing one grid point's polarisations (1 or 2)
     int sort_chunks;                      // -1 auto (grid larger than L2), 0 off, 1 on
-    int sample_order;                     // grid_plan_set_sample_order: -1 auto, 0 input order, 1 sorted by grid cell
+    int sample_order;                     // grid_plan_set_sample_order: -1 auto, 0 input order, 1 sorted by grid cell, 2 sorted and kept
+    int order_kept;                       // mode 2: the workspace holds the sorted records of the current samples
     int n_sm, max_smem;
     int last_launches;
     int user_tuned;                       // set_tuning / set_pol_split was called: set_samples keeps the block
@@ -257,7 +258,11 @@ int padded_support(int S, int N, int W, int O) {
 bool is_padded(const grid_plan* p) { return p->Sk != p->S; }
 int tap_rows(const grid_plan* p) { return p->W * p->O * (is_padded(p) ? 2 : 1); }
 
-size_t records_bytes(const grid_plan* p) { return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec); }
+bool cell_sort_on(const grid_plan* p);
+// 16 bytes per sample; in cell order every record has a 32-byte sector of its own (kCellRecStride, cell_sort.cuh)
+size_t records_bytes(const grid_plan* p) {
+    return (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(SampleRec) * (cell_sort_on(p) ? kCellRecStride : 1);
+}
 
 // workspace: [256 B counters][order bins][records][chunk order]
 constexpr size_t kHeadBytes = 256 + 2 * kOrderBins * sizeof(uint32_t);
@@ -620,6 +625,7 @@ static void retune(grid_plan* plan) {
 int grid_plan_set_samples(grid_plan* plan, long long n_vis) {
     if (!plan || n_vis < 0) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_samples: invalid argument");
     plan->n_vis = n_vis;
+    plan->order_kept = 0;
     retune(plan);
     return GRID_OK;
 }
@@ -641,6 +647,7 @@ int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes) {
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_workspace: null or misaligned pointer");
     plan->workspace = dev_ptr;
     plan->workspace_bytes = bytes;
+    plan->order_kept = 0;
     return GRID_OK;
 }
 
@@ -671,6 +678,7 @@ int grid_plan_set_tuning(grid_plan* plan, int variant, int cu, int cv, int threa
     if (rc != GRID_OK) return rc;
     *plan = trial;
     plan->user_tuned = 1;
+    plan->order_kept = 0;
     return GRID_OK;
 }
 
@@ -810,6 +818,7 @@ int grid_plan_set_pol_split(grid_plan* plan, int lanes) {
     if (rc != GRID_OK) return rc;
     *plan = trial;
     plan->user_tuned = 1;
+    plan->order_kept = 0;
     return GRID_OK;
 }
 
@@ -827,8 +836,9 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode) {
 }
 
 int grid_plan_set_sample_order(grid_plan* plan, int mode) {
-    if (!plan || mode < -1 || mode > 1) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_sample_order: mode must be -1, 0 or 1");
-    if (mode == 1 && plan->variant != 3)
+    if (!plan || mode < -1 || mode > 2) return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_sample_order: mode must be -1, 0, 1 or 2");
+    plan->order_kept = 0;
+    if (mode >= 1 && plan->variant != 3)
         return fail(GRID_ERR_UNSUPPORTED, "grid_plan_set_sample_order: cell order needs the warp kernel (variant 3)");
     plan->sample_order = mode;
     retune(plan);
@@ -893,7 +903,10 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     // reset the chunk queue and the hop statistics, then a1: quantise pass
     if (cudaMemsetAsync(counters, 0, kHeadBytes, stream) != cudaSuccess)
         return fail(GRID_ERR_CUDA, "grid_execute: %s", cudaGetErrorString(cudaGetLastError()));
-    if (sorted) {
+    // mode 2: the caller guarantees the same uvw and weights as in the call that sorted them -- the records are reused
+    const bool keep = sorted && plan->sample_order == 2;
+    if (sorted && keep && plan->order_kept) {
+    } else if (sorted) {
         unsigned char* scratch = reinterpret_cast<unsigned char*>(plan->workspace) + cell_sort_offset(plan);
         uint32_t* hist = reinterpret_cast<uint32_t*>(scratch);
         uint32_t* sums = reinterpret_cast<uint32_t*>(scratch + cell_sums_offset(plan));
@@ -908,13 +921,14 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
         cell_scan_reduce_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
         cell_scan_sums_kernel<<<1, 1024, 0, stream>>>(sums, (int)scan_blocks);
         cell_scan_apply_kernel<<<scan_blocks, 256, 0, stream>>>(hist, sums);
-        if (plan->P == 1 && !degrid_out)           // degridding needs the sample's index: where its result goes
+        if (plan->P == 1 && !degrid_out && !keep)  // degridding needs the sample's index (where its result goes), kept records too
             cell_scatter_kernel<true><<<blocks, 256, 0, stream>>>(uvw, weights, reinterpret_cast<const float2*>(vis), n_vis, qp,
                                                                   hist, ranks, reinterpret_cast<uint4*>(recs));
         else
             cell_scatter_kernel<false><<<blocks, 256, 0, stream>>>(uvw, weights, nullptr, n_vis, qp, hist, ranks,
                                                                    reinterpret_cast<uint4*>(recs));
         plan->last_launches += 5;
+        plan->order_kept = keep ? 1 : 0;
     } else if (!ext_recs) {
         const long long threads = (n_vis + 3) / 4;
         const long long blocks = (threads + 255) / 256;
@@ -933,7 +947,8 @@ static int execute_impl(grid_plan* plan, const float* uvw, const void* ext_recs,
     gp.vis_out = reinterpret_cast<float2*>(degrid_out);
     gp.counters = counters;
     gp.rec16 = (plan->variant == 3 && !ext_recs) ? 1 : 0;
-    gp.sorted = sorted ? 1 : 0;
+    gp.sorted = !sorted ? 0 : (plan->P == 1 && !degrid_out && !keep) ? 1 : 2;   // 1: records carry weight * vis, 2: {weight, index}
+    gp.sorted_stride = kCellRecStride;
     gp.n_vis = n_vis;
     gp.N = plan->N; gp.S = plan->variant == 3 ? plan->Sk : plan->S;
     gp.n_rows = plan->variant == 3 ? tap_rows(plan) : plan->W * plan->O;
@@ -1134,6 +1149,7 @@ int grid_compress(grid_plan* plan, const float* uvw, const float* vis, const flo
     cudaStream_t stream = (cudaStream_t)stream_;
     if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_compress: null plan");
     plan->last_launches = 0;
+    plan->order_kept = 0;                            // the records of this call overwrite the workspace
     if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_compress: call grid_plan_set_samples first");
     if (plan->variant != 3) return fail(GRID_ERR_UNSUPPORTED, "grid_compress: power-of-two supports (variant 3) only");
     if (!out_count) return fail(GRID_ERR_INVALID_ARG, "grid_compress: null out_count");
@@ -1203,12 +1219,14 @@ int grid_degrid(grid_plan* plan, const float* uvw, const float* weights, const f
                 const int rc = execute_impl(&tmp, uvw, nullptr, plan->n_vis, nullptr, weights, conv_kernel,
                                             const_cast<float*>(grid), stream, vis_out);
                 plan->last_launches = tmp.last_launches;
+                plan->order_kept = tmp.order_kept;   // gridding and degridding share the kept records
                 return rc;
             }
         }
         g_err[0] = 0;                                // no coarsened kernel for this shape: gather below
     }
     const long long n = plan->n_vis;
+    plan->order_kept = 0;                            // the gather kernel's records overwrite the workspace
     if (n * 32 / 256 + 1 > 0x7fffffffLL) return fail(GRID_ERR_UNSUPPORTED, "grid_degrid: too many samples");
     unsigned int* counters = reinterpret_cast<unsigned int*>(plan->workspace);
     CycRec* recs = reinterpret_cast<CycRec*>(reinterpret_cast<unsigned char*>(plan->workspace) + kHeadBytes);
@@ -1239,6 +1257,7 @@ static int execute_dense_impl(grid_plan* plan, const float* uvw, const float* vi
     cudaStream_t stream = (cudaStream_t)stream_;
     if (!plan) return fail(GRID_ERR_INVALID_ARG, "grid_execute_dense: null plan");
     plan->last_launches = 0;
+    plan->order_kept = 0;                            // the records of this call overwrite the workspace
     if (plan->n_vis < 0) return fail(GRID_ERR_STATE, "grid_execute_dense: call grid_plan_set_samples first");
     if (plan->n_vis == 0) return GRID_OK;
     if (!uvw || !vis || !weights || !conv_kernel_2d || !grid)

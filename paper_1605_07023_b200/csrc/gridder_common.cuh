@@ -60,8 +60,9 @@ struct GridParams {
     long long dense_pol_stride;   // dense GCF per polarisation: elements between the tables of two polarisations
     int tap_pad;              // warp kernel: zero taps added to each row (support padded to a power of two)
     int rec16;                // warp kernel: records are 16 bytes {pos, rows, weight, -} (quantise format 2), else CycRec
-    int sorted;               // warp kernel: recs are in cell order (cell_sort.cuh): {pos, rows, weight, sample index}, or
-                              // for one polarisation {pos, rows, weight * vis}; chunks are contiguous runs of them
+    int sorted_stride;        // cell order: records are this many 16-byte units apart
+    int sorted;               // warp kernel: recs are in cell order (cell_sort.cuh), chunks are contiguous runs of them:
+                              // 2 = {pos, rows, weight, sample index}, 1 = one polarisation, {pos, rows, weight * vis}
 };
 
 }  // namespace gridb200

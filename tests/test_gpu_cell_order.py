@@ -176,3 +176,53 @@ def test_adjoint_identity_in_cell_order(oracle_mod):
     lhs = np.vdot(gridded.astype(np.complex128), G.astype(np.complex128))          # as in tests/test_gpu_degrid.py
     rhs = np.vdot(vis.astype(np.complex128), degridded.astype(np.complex128))
     assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
+
+
+@pytest.mark.parametrize("P", [1, 4])
+def test_cell_order_kept_across_calls(oracle_mod, P):
+    # grid_plan_set_sample_order(plan, 2): the first call sorts, later calls with the SAME uvw and weights reuse the
+    # sorted records (one launch), whatever the visibilities are; degridding shares them; changing the samples re-sorts
+    import torch
+    from paper_1605_07023_b200 import binding
+    N, S, O, W, n = 160, 8, 4, 2, 30_011
+    uvw, vis, wts, kernel = synth.random_problem(8700 + P, n, N, S, O, W, P, spread=0.5, walk=1.3)
+    uvw[500:520, 0] = np.nan
+    vis2 = (vis * (0.3 - 0.7j) + 1.0).astype(np.complex64)
+    dev = torch.device("cuda:0")
+    d = {k: torch.from_numpy(np.ascontiguousarray(v)).to(dev) for k, v in
+         dict(uvw=uvw, vis=vis, vis2=vis2, wts=wts, kernel=kernel).items()}
+    plan = binding.GridPlan(N, S, O, W, P)
+    try:
+        plan.set_samples(n)
+        plan.set_sample_order(2)
+        plan.allocate_workspace(dev)
+        assert plan.info()["sample_order"] == 1
+        g1 = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+        plan.execute(d["uvw"], d["vis"], d["wts"], d["kernel"], g1)
+        assert plan.last_launches() == 6
+        g2 = torch.zeros_like(g1)
+        plan.execute(d["uvw"], d["vis2"], d["wts"], d["kernel"], g2)
+        assert plan.last_launches() == 1                          # the gridding kernel alone
+        torch.cuda.synchronize()
+        assert_parity(g1.cpu().numpy(), oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel), "first call")
+        assert_parity(g2.cpu().numpy(), oracle_mod.grid(N, S, O, W, P, uvw, vis2, wts, kernel), "kept order, new visibilities")
+        # degridding walks the same records
+        rng = np.random.default_rng(P)
+        G = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+        out = plan.degrid(d["uvw"], d["wts"], d["kernel"], torch.from_numpy(G).to(dev))
+        assert plan.last_launches() <= 2, plan.last_launches()    # (+ a memset-free kernel only; no sort)
+        torch.cuda.synchronize()
+        ref = oracle_mod.degrid(N, S, O, W, P, uvw, wts, kernel, G)
+        got = out.cpu().numpy().astype(np.complex128)
+        assert np.linalg.norm(got - ref) <= 1e-5 * np.linalg.norm(ref)
+        # new samples: the records are dropped and rebuilt
+        m = n - 1001
+        plan.set_samples(m)
+        plan.allocate_workspace(dev)
+        g3 = torch.zeros_like(g1)
+        plan.execute(d["uvw"][:m].contiguous(), d["vis"][:m].contiguous(), d["wts"][:m].contiguous(), d["kernel"], g3)
+        assert plan.last_launches() == 6
+        torch.cuda.synchronize()
+        assert_parity(g3.cpu().numpy(), oracle_mod.grid(N, S, O, W, P, uvw[:m], vis[:m], wts[:m], kernel), "after set_samples")
+    finally:
+        plan.destroy()

@@ -204,7 +204,9 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode);
  *       grid_plan_set_sample_order(plan, 2) again after changing uvw or weights in place.  The workspace must not be
  *       shared with another plan meanwhile.
  *   0 = input order (chunks of the caller's baseline-major order, walked as grid_plan_set_traversal says).
- *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, else input order.
+ *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, unless the layout hint says
+ *       the samples are single-channel tracks (they move a fraction of a cell per sample as they come);
+ *       else input order.
  * Applies to grid_execute and grid_degrid (whose results then go back to their samples' places through the index in
  * the record); grid_execute_static, grid_execute_compressed (its input is already ordered by the caller) and
  * grid_execute_dense* always use input order. */

@@ -285,6 +285,9 @@ bool cell_sort_possible(const grid_plan* p) {
 bool cell_sort_on(const grid_plan* p) {
     if (p->sample_order == 0 || !cell_sort_possible(p)) return false;
     if (p->sample_order > 0) return true;
+    // single-channel tracks (the paper's data) move a fraction of a cell per sample in input order:
+    // nothing to gain (paper-shaped S = 32, P = 4: 6.07 ms in input order, 6.36 ms sorted)
+    if (p->n_channels == 1 && (long long)p->n_baselines * p->n_times == p->n_vis) return false;
     return p->n_vis >= kCellSortMinSamples && (long long)p->N * p->N <= 8 * p->n_vis;
 }
 size_t cell_hist_entries(const grid_plan* p) {
@@ -634,6 +637,8 @@ int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_ch
     if (!plan || n_baselines < 0 || n_times < 0 || n_channels < 0)
         return fail(GRID_ERR_INVALID_ARG, "grid_plan_set_layout: invalid argument");
     plan->n_baselines = n_baselines; plan->n_times = n_times; plan->n_channels = n_channels;
+    plan->order_kept = 0;
+    retune(plan);                                    // the automatic sample order looks at the layout
     return GRID_OK;
 }
 

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cmath>
 #include <new>
 
 #include "grid_kernel.cuh"
@@ -540,13 +541,15 @@ __device__ __forceinline__ float tune_unit(uint32_t a, uint32_t b) { return (tun
 
 __global__ void __launch_bounds__(256)
 tune_fill_kernel(float* __restrict__ uvw, float2* __restrict__ vis, float* __restrict__ weights, long long n, int P,
-                 int N, int S, int W, int n_times, int n_chan, unsigned int seed) {
+                 int N, int S, int W, int n_times, int n_chan, unsigned int seed, float extent) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     const long long row = k / n_chan;
     const int c = (int)(k - row * n_chan), t = (int)(row % n_times);
     const uint32_t b = (uint32_t)(row / n_times);
-    const float rmax = 0.45f * N - S, rmin = fminf(0.02f * N, rmax);
+    // extent < 1 (cell order): the tracks cover that fraction of the grid's width, so that the synthetic set has as
+    // many samples per grid cell as the caller's input -- which is what decides how often a sorted walk moves
+    const float rmax = fmaxf((0.45f * N - S) * extent, 2.f), rmin = fminf(0.02f * N * extent, rmax);
     const float r = rmin * __powf(rmax / rmin, tune_unit(seed, 3 * b));            // log-uniform radius
     const float th0 = 6.2831853f * tune_unit(seed, 3 * b + 1);
     const float th = th0 + 1.0471976f * (t - 0.5f * n_times) / (n_times > 1 ? n_times : 1);   // 60 degrees over the track
@@ -731,6 +734,12 @@ int grid_plan_autotune(grid_plan* plan, long long n_samples, unsigned int seed, 
 
     grid_plan t = *plan;                                         // a private plan: the caller's stays untouched until the end
     t.n_vis = n; t.n_baselines = (int)n_bl; t.n_times = n_times; t.n_channels = n_chan;
+    // tune in the sample order the caller's plan will grid in (the synthetic set is smaller than the real input and
+    // would not always get the same automatic choice)
+    if (plan->n_vis > 0) t.sample_order = cell_sort_on(plan) ? 1 : 0;
+    t.order_kept = 0;
+    float extent = 1.f;
+    if (cell_sort_on(&t) && plan->n_vis > n) extent = sqrtf((float)n / (float)plan->n_vis);
     t.ev_start = t.ev_stop = nullptr;
     const size_t grid_bytes = (size_t)plan->N * plan->N * plan->P * sizeof(float2);
     const size_t kern_bytes = (size_t)plan->W * plan->O * plan->S * sizeof(float2);
@@ -756,7 +765,7 @@ int grid_plan_autotune(grid_plan* plan, long long n_samples, unsigned int seed, 
     }
     t.workspace = d_ws;
     tune_fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(d_uvw, d_vis, d_w, n, plan->P, plan->N, plan->S, plan->W,
-                                                                     n_times, n_chan, seed);
+                                                                     n_times, n_chan, seed, extent);
     tune_taps_kernel<<<(unsigned)(((long long)plan->W * plan->O * plan->S + 255) / 256), 256, 0, stream>>>(d_kern, plan->W * plan->O, plan->S);
     cudaMemsetAsync(d_grid, 0, grid_bytes, stream);
     for (int k = 0; k < n_cand && rc == GRID_OK; ++k) {

@@ -228,7 +228,9 @@ int grid_plan_set_pol_split(grid_plan* plan, int lanes);
  *
  * grid_plan_autotune: synthesises n_samples samples on the device (0 = 1 << 20; tracks of a synthetic array
  * shaped by the layout hint if one is set, else single-channel tracks; counter-based generator seeded with
- * `seed`; random visibilities and weights, Kaiser-Bessel-like taps), grids them with every candidate onto a
+ * `seed`; random visibilities and weights, Kaiser-Bessel-like taps; where the plan grids in cell order the tracks
+ * are confined to a part of the grid so that the set has the plan's samples per grid cell), grids them -- in the
+ * plan's sample order -- with every candidate onto a
  * scratch grid of the plan's size (cudaMalloc'ed and freed here, like the inputs), times each with CUDA events on
  * `stream` (second of two runs) and installs the fastest (as grid_plan_set_tuning + grid_plan_set_pol_split
  * would).  Synchronises `stream`.  results, if not NULL, receives for every candidate, in the order of

@@ -513,6 +513,8 @@ QuantParams quant_params(const grid_plan* p) {
     q.format = p->variant == 3 ? 2 : 0;
     q.c_centre = (double)p->O * (double)(p->N / 2) + 0.5;
     q.oversample = p->O;
+    q.o_shift = -1;
+    for (int k = 0; k < 16; ++k) if ((1 << k) == p->O) q.o_shift = k;
     q.shift = p->O - (p->O * p->S + 1) / 2;
     q.q_limit = (p->N - p->S + 1) * p->O;
     q.n_wplanes = p->W;

@@ -25,6 +25,7 @@ struct QuantParams {
     int format;           // 0: SampleRec (16 B), 1: CycRec (8 B), 2: CycRec + weight (16 B: pos, rows, weight, 0)
     double c_centre;      // O*floor(N/2) + 0.5
     int oversample;       // O
+    int o_shift;          // log2(O) if O is a power of two, else -1
     int shift;            // O - ceil(O*S/2)
     int q_limit;          // (N-S+1)*O : valid iff 0 <= q < q_limit
     int n_wplanes;

@@ -16,7 +16,8 @@ __device__ __forceinline__ bool quantise_axis(float x, const QuantParams& qp, in
     const bool ok = (q >= 0.0 && q < (double)qp.q_limit);        // false for NaN, Inf, outside the grid
     // skipped samples still get in-grid coordinates (fmax/fmin drop NaN): the bin == support kernel walks them
     const int qi = (int)fmin(fmax(q, 0.0), (double)(qp.q_limit - 1));
-    const int c = qi / qp.oversample;
+    // oversampling factors are powers of two in practice: a shift instead of a ~20-instruction division sequence
+    const int c = qp.o_shift >= 0 ? (qi >> qp.o_shift) : qi / qp.oversample;
     *cell = c;
     *sub = qi - c * qp.oversample;
     return ok;

@@ -168,3 +168,53 @@ def test_autotune_needs_a_device(binding):
         plan.autotune(stream=0)                        # the default stream by handle: torch has no device to ask
     assert e.value.code == binding.GRID_ERR_CUDA       # no CPU fallback, no silent success
     plan.destroy()
+
+
+def test_sample_order_host_logic(binding):
+    # grid_plan_set_sample_order (include/grid.h): the automatic rule, the workspace it needs, the block it selects
+    def plan(N, S, P, n, layout=None, W=1):
+        p = binding.GridPlan(N, S, 8, W, P)
+        p.set_samples(n)
+        if layout:
+            p.set_layout(*layout)
+        return p
+    big = 2016 * 256 * 64
+    p = plan(2048, 8, 4, big, (2016, 256, 64))
+    try:
+        assert p.info()["sample_order"] == 1                              # large multi-channel input: cell order
+        ws_cell = p.workspace_bytes()
+        assert (p.info()["cu"], p.info()["cv"], p.info()["pol_split"]) == (2, 2, 1)
+        p.set_sample_order(0)
+        assert p.info()["sample_order"] == 0
+        ws_input = p.workspace_bytes()
+        # 4 bytes per grid cell (+ 1, rounded to the scan tile) + 16 more bytes per record + 4 per rank, and change
+        extra = ws_cell - ws_input
+        assert 4 * 2048 * 2048 + 20 * big <= extra <= 4 * 2048 * 2048 + 20 * big + (1 << 20), extra
+        p.set_sample_order(2)
+        assert p.info()["sample_order"] == 1 and p.workspace_bytes() == ws_cell
+        with pytest.raises(binding.GridError):
+            p.set_sample_order(3)
+    finally:
+        p.destroy()
+    for args, want in (((2048, 8, 4, (1 << 20) - 1), 0),                  # small input: the extra launches do not pay
+                       ((2048, 8, 4, 1 << 20), 1),
+                       ((8192, 8, 4, 1 << 22), 0),                        # histogram of 67 M cells for 4 M samples
+                       ((8192, 8, 4, 1 << 23), 1),
+                       ((4096, 32, 4, 64 * 63 // 2 * 3600, (2016, 3600, 1)), 0),   # single-channel tracks (the paper's data)
+                       ((4096, 32, 4, 64 * 63 // 2 * 3600), 1),
+                       ((4096, 16, 1, 33_030_144, (2016, 128, 128), 32), 1)):
+        p = plan(*args)
+        try:
+            assert p.info()["sample_order"] == want, (args, p.info())
+        finally:
+            p.destroy()
+    # the scatter and padded kernels have no cell order
+    p = plan(2048, 8, 4, big)
+    try:
+        p.set_sample_order(0)
+        p.set_tuning(variant=1, cu=2, cv=2, threads_per_cta=256, batch=32, chunk=256)
+        with pytest.raises(binding.GridError):
+            p.set_sample_order(1)
+        assert p.info()["sample_order"] == 0
+    finally:
+        p.destroy()

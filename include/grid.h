@@ -207,9 +207,9 @@ int grid_plan_set_chunk_order(grid_plan* plan, int mode);
  *  -1 = automatic (default): cell order when n_vis >= 2^20 and grid_size^2 <= 8 n_vis, unless the layout hint says
  *       the samples are single-channel tracks (they move a fraction of a cell per sample as they come);
  *       else input order.
- * Applies to grid_execute and grid_degrid (whose results then go back to their samples' places through the index in
- * the record); grid_execute_static, grid_execute_compressed (its input is already ordered by the caller) and
- * grid_execute_dense* always use input order. */
+ * Applies to grid_execute, grid_execute_dense* (coarsened kernel) and grid_degrid (whose results then go back to their
+ * samples' places through the index in the record); grid_execute_static and grid_execute_compressed (its input is
+ * already ordered by the caller) always use input order. */
 int grid_plan_set_sample_order(grid_plan* plan, int mode);
 
 /* Variant 3, n_pol = 4: spread the polarisations of one grid point over `lanes` adjacent threads

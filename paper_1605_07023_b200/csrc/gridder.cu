@@ -281,7 +281,7 @@ size_t tap_table_bytes(const grid_plan* p) {
 // input itself (a sparse input on a huge grid would spend its time scanning empty cells).
 constexpr long long kCellSortMinSamples = 1 << 20;
 bool cell_sort_possible(const grid_plan* p) {
-    return p->variant == 3 && !p->dense && p->n_vis > 0 && p->n_vis < 0x7fffffffLL;
+    return p->variant == 3 && p->n_vis > 0 && p->n_vis < 0x7fffffffLL;
 }
 bool cell_sort_on(const grid_plan* p) {
     if (p->sample_order == 0 || !cell_sort_possible(p)) return false;
@@ -1292,6 +1292,7 @@ static int execute_dense_impl(grid_plan* plan, const float* uvw, const float* vi
         if (tmp.P == 1) { tmp.cu = logs == 2 ? 2 : (logs == 5 ? 8 : 4); tmp.cv = logs == 2 ? 2 : 4; }
         else if (tmp.P == 2) { tmp.cu = logs == 2 ? 2 : 4; tmp.cv = 2; }
         else { tmp.cu = logs <= 3 ? 2 : 4; tmp.cv = 2; }
+        if (!cell_sort_on(plan)) tmp.sample_order = 0;   // cell order only where the caller's workspace provides for it
         if (derive(&tmp) == GRID_OK) {               // uses a subset of the plan's workspace (no tap table copy)
             const int rc = execute_impl(&tmp, uvw, nullptr, plan->n_vis, vis, weights, conv_kernel_2d, grid, stream);
             plan->last_launches = tmp.last_launches;

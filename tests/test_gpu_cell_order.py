@@ -226,3 +226,35 @@ def test_cell_order_kept_across_calls(oracle_mod, P):
         assert_parity(g3.cpu().numpy(), oracle_mod.grid(N, S, O, W, P, uvw[:m], vis[:m], wts[:m], kernel), "after set_samples")
     finally:
         plan.destroy()
+
+
+@pytest.mark.parametrize("S,P,W,per_pol", [(8, 4, 2, False), (8, 1, 3, False), (16, 1, 2, False), (32, 4, 1, False),
+                                           (16, 2, 2, True), (8, 4, 1, True)])
+def test_dense_gcf_in_cell_order(oracle_mod, S, P, W, per_pol):
+    # grid_execute_dense / grid_execute_dense_pol walk the sorted records too (one polarisation: the record carries
+    # the pre-weighted visibility)
+    import torch
+    from paper_1605_07023_b200 import binding
+    N, O, n = 200, 3, 12_007
+    uvw, vis, wts, _ = synth.random_problem(8900 + S + P, n, N, S, O, W, P, spread=0.5, walk=1.2)
+    uvw[10:20, 1] = np.nan
+    vis[10:20] = np.inf
+    rng = np.random.default_rng(S * 7 + P)
+    shape = ((P,) if per_pol else ()) + (W, O, O, S, S)
+    k2 = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    ref = (oracle_mod.grid_dense_pol if per_pol else oracle_mod.grid_dense)(N, S, O, W, P, uvw, vis, wts, k2)
+    dev = torch.device("cuda:0")
+    plan = binding.GridPlan(N, S, O, W, P)
+    try:
+        plan.set_samples(n)
+        plan.set_sample_order(1)
+        plan.allocate_workspace(dev)
+        grid = torch.zeros((N, N, P), dtype=torch.complex64, device=dev)
+        call = plan.execute_dense_pol if per_pol else plan.execute_dense
+        call(torch.from_numpy(uvw).to(dev), torch.from_numpy(np.ascontiguousarray(vis)).to(dev).reshape(n, P),
+             torch.from_numpy(wts).to(dev), torch.from_numpy(k2).to(dev), grid)
+        torch.cuda.synchronize()
+        assert plan.last_launches() == 6, plan.last_launches()      # the sort's five kernels + the dense kernel
+        assert_parity(grid.cpu().numpy(), ref, f"dense in cell order S={S} P={P} W={W} per_pol={per_pol}")
+    finally:
+        plan.destroy()

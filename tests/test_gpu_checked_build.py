@@ -3,7 +3,7 @@ measurement pool ("runs under it have left GPUs needing a reset"), so the kernel
 forms (atomic flushes, sample gathers, degridding stores) and every shared-memory slot it indexes (raw ring, cooked
 arrays, tap table) is tested against its bounds; violations are counted, the access suppressed.  This test runs the
 checked library in a subprocess on the shapes that exercise each code path -- several teams per warp, multi-warp teams
-(S = 64), tiles (S = 128), padded supports, taps in global memory, both traversals, ragged tails, off-grid samples,
+(S = 64), tiles (S = 128), padded supports, taps in global memory, both traversals and cell order, ragged tails, off-grid samples,
 footprints in the grid's corners -- and requires zero violations AND parity with the oracle.  (Races between the
 groups' rings are not covered by this; the ring protocol is two named barriers per batch, grid_warp_kernel.cuh.)"""
 import json
@@ -29,7 +29,7 @@ out = []
 cases = [(8, 4, 8, 1, None), (16, 1, 8, 32, None), (7, 1, 8, 1, None), (4, 4, 4, 3, None), (64, 2, 2, 2, None),
          (128, 1, 2, 2, None), (32, 4, 8, 300, None), (13, 2, 4, 2, None), (8, 4, 8, 1, dict(pol_split=2))]
 for S, P, O, W, extra in cases:
-    for mode in (0, 1):
+    for mode in (0, 1, 2):                       # channel-innermost, time-innermost, cell order (cell_sort.cuh)
         N = 640 if S >= 64 else 256
         cfg = synth.shrink(synth.get_config("cfg1"), n_ant=8, n_times=37, n_chan=11, grid_size=N)
         rng = np.random.default_rng(S + P)
@@ -43,7 +43,9 @@ for S, P, O, W, extra in cases:
         wts = rng.uniform(0.5, 1, n).astype(np.float32)
         kern = (rng.standard_normal((W, O, S)) + 1j * rng.standard_normal((W, O, S))).astype(np.complex64)
         plan = binding.GridPlan(N, S, O, W, P)
-        plan.set_samples(n); plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan); plan.set_traversal(mode, 16)
+        plan.set_samples(n); plan.set_layout(cfg.n_baselines, cfg.n_times, cfg.n_chan)
+        if mode < 2: plan.set_traversal(mode, 16)
+        else: plan.set_sample_order(1)
         if extra: plan.set_pol_split(extra["pol_split"])
         plan.set_tuning(batch=8, chunk=40)
         plan.allocate_workspace(dev)
@@ -57,6 +59,7 @@ for S, P, O, W, extra in cases:
         c2 = plan.debug_counters()
         ref = oracle.degrid(N, S, O, W, P, uvw, wts, kern, g_in.cpu().numpy())
         drel = float(np.linalg.norm(vo.cpu().numpy() - ref) / np.linalg.norm(ref))
+        assert plan.info()["sample_order"] == (1 if mode == 2 else 0)
         out.append(dict(S=S, P=P, W=W, mode=mode, variant=plan.info()["variant"], grid_counters=c1, degrid_counters=c2,
                         rel=float(rel), max_abs=float(mx), degrid_rel=drel))
         plan.destroy()
@@ -76,7 +79,7 @@ def test_checked_build_reports_no_violation():
     assert r.returncode == 0 and lines, (r.returncode, r.stdout[-1000:], r.stderr[-3000:])
     line = lines[-1]
     res = json.loads(line[len("RESULT "):])
-    assert len(res) == 18
+    assert len(res) == 27
     for e in res:
         assert e["variant"] == 3, e
         assert e["grid_counters"] == [0] * 8 and e["degrid_counters"] == [0] * 8, e

@@ -60,20 +60,17 @@ cell_count_kernel(const float* __restrict__ uvw, long long n, QuantParams qp, ui
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const bool have = first + k < n;
-        uint32_t key = nn;
+        uint32_t key = 0xffffffffu;                    // no sample: a group of its own, nothing counted
         if (have) key = cell_key(make_cyc_record(quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp), qp), N, nn);
-        rk[k] = 0;
-        if (have && key != nn) rk[k] = atomicAdd(hist + key, 1u);
-        // skipped samples share one bin: one atomic per warp (an input that is mostly off the grid would
-        // otherwise serialise on it)
-        const uint32_t inv = __ballot_sync(0xffffffffu, have && key == nn);
-        if (inv) {
-            const int leader = __ffs(inv) - 1;
-            uint32_t base = 0;
-            if ((int)lane == leader) base = atomicAdd(hist + nn, (uint32_t)__popc(inv));
-            base = __shfl_sync(0xffffffffu, base, leader);
-            if (have && key == nn) rk[k] = base + (uint32_t)__popc(inv & ((1u << lane) - 1u));
-        }
+        // One atomic per warp and distinct cell: the lanes that hit the same cell (neighbouring channels of a short
+        // baseline; all the skipped samples, which share the bin nn) take consecutive ranks from one atomicAdd.  An
+        // input concentrated on few cells would otherwise serialise on their counters.
+        const uint32_t peers = __match_any_sync(0xffffffffu, key);
+        const int leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if (have && (int)lane == leader) base = atomicAdd(hist + key, (uint32_t)__popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        rk[k] = base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
     }
     if (first + 4 <= n) *reinterpret_cast<uint4*>(ranks + first) = make_uint4(rk[0], rk[1], rk[2], rk[3]);
     else {

@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(256) cell_scan_reduce_kernel(const uint32_t* _
     if (threadIdx.x == 0) sums[blockIdx.x] = ws[0] + ws[1] + ws[2] + ws[3] + ws[4] + ws[5] + ws[6] + ws[7];
 }
 
-// exclusive scan of the block sums, one block of 1024 threads, carried over slabs of 1024
+// exclusive scan of the block sums, one block of 1024 threads, carried over slabs of 1024; sums[nb] = the total
 __global__ void __launch_bounds__(1024) cell_scan_sums_kernel(uint32_t* __restrict__ sums, int nb) {
     __shared__ uint32_t ws[32];
     __shared__ uint32_t carry;
@@ -128,10 +128,13 @@ __global__ void __launch_bounds__(1024) cell_scan_sums_kernel(uint32_t* __restri
         if (t == 1023) carry = incl;
         __syncthreads();
     }
+    if (t == 0) sums[nb] = carry;
 }
 
 __global__ void __launch_bounds__(256) cell_scan_apply_kernel(uint32_t* __restrict__ hist, const uint32_t* __restrict__ sums) {
     __shared__ uint32_t ws[8];
+    // a tile without samples: nobody will ask for its offsets (on a large, sparsely covered grid most tiles are empty)
+    if (__ldg(sums + blockIdx.x + 1) == __ldg(sums + blockIdx.x)) return;
     uint32_t v[kScanPerThread];
     uint32_t* p = hist + (size_t)blockIdx.x * kScanTile + threadIdx.x * kScanPerThread;
     const uint32_t mine = scan_load16(p, v);

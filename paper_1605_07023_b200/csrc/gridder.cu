@@ -297,7 +297,7 @@ size_t cell_hist_entries(const grid_plan* p) {
 // [histogram / offsets][block sums][ranks]
 size_t cell_sums_offset(const grid_plan* p) { return cell_hist_entries(p) * sizeof(uint32_t); }
 size_t cell_ranks_offset(const grid_plan* p) {
-    return cell_sums_offset(p) + ((cell_hist_entries(p) / kScanTile * sizeof(uint32_t) + 255) & ~(size_t)255);
+    return cell_sums_offset(p) + (((cell_hist_entries(p) / kScanTile + 1) * sizeof(uint32_t) + 255) & ~(size_t)255);
 }
 size_t cell_sort_bytes(const grid_plan* p) {
     return cell_sort_on(p) ? cell_ranks_offset(p) + (size_t)((p->n_vis + 3) / 4 * 4) * sizeof(uint32_t) : 0;

@@ -34,7 +34,7 @@ static constexpr int kScanTile = 256 * kScanPerThread;        // histogram entri
 __device__ __forceinline__ void load_uvw4(const float* __restrict__ uvw, long long first, long long n, float (&c)[12]) {
     if (first + 4 <= n) {
         const float4* p = reinterpret_cast<const float4*>(uvw + first * 3);
-        const float4 a = __ldg(p), b = __ldg(p + 1), d = __ldg(p + 2);
+        const float4 a = __ldcs(p), b = __ldcs(p + 1), d = __ldcs(p + 2);       // streamed once: do not displace the histogram
         c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z;
         c[7] = b.w; c[8] = d.x; c[9] = d.y; c[10] = d.z; c[11] = d.w;
     } else {
@@ -72,7 +72,7 @@ cell_count_kernel(const float* __restrict__ uvw, long long n, QuantParams qp, ui
         base = __shfl_sync(0xffffffffu, base, leader);
         rk[k] = base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
     }
-    if (first + 4 <= n) *reinterpret_cast<uint4*>(ranks + first) = make_uint4(rk[0], rk[1], rk[2], rk[3]);
+    if (first + 4 <= n) __stcs(reinterpret_cast<uint4*>(ranks + first), make_uint4(rk[0], rk[1], rk[2], rk[3]));
     else {
 #pragma unroll
         for (int k = 0; k < 4; ++k) if (first + k < n) ranks[first + k] = rk[k];
@@ -173,12 +173,12 @@ cell_scatter_kernel(const float* __restrict__ uvw, const float* __restrict__ wei
     uint32_t rk[4] = {0u, 0u, 0u, 0u};
     float2 v[4];
     if (first + 4 <= n) {
-        const float4 w4 = __ldg(reinterpret_cast<const float4*>(weights + first));
+        const float4 w4 = __ldcs(reinterpret_cast<const float4*>(weights + first));
         w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
-        const uint4 r4 = __ldg(reinterpret_cast<const uint4*>(ranks + first));
+        const uint4 r4 = __ldcs(reinterpret_cast<const uint4*>(ranks + first));
         rk[0] = r4.x; rk[1] = r4.y; rk[2] = r4.z; rk[3] = r4.w;
         if constexpr (P1) {
-            const float4 a = __ldg(reinterpret_cast<const float4*>(vis + first)), b = __ldg(reinterpret_cast<const float4*>(vis + first) + 1);
+            const float4 a = __ldcs(reinterpret_cast<const float4*>(vis + first)), b = __ldcs(reinterpret_cast<const float4*>(vis + first) + 1);
             v[0] = make_float2(a.x, a.y); v[1] = make_float2(a.z, a.w); v[2] = make_float2(b.x, b.y); v[3] = make_float2(b.z, b.w);
         }
     } else {
@@ -197,9 +197,10 @@ cell_scatter_kernel(const float* __restrict__ uvw, const float* __restrict__ wei
             const CycRec r = make_cyc_record(quantise_sample(c[3 * k], c[3 * k + 1], c[3 * k + 2], qp), qp);
             const uint32_t at = __ldg(offsets + cell_key(r, N, nn)) + rk[k];
             uint4* dst = out + (size_t)at * kCellRecStride;
-            if constexpr (P1) dst[0] = make_uint4(r.pos, r.rows, __float_as_uint(v[k].x * w[k]), __float_as_uint(v[k].y * w[k]));
-            else dst[0] = make_uint4(r.pos, r.rows, __float_as_uint(w[k]), (uint32_t)(first + k));
-            dst[1] = make_uint4(0u, 0u, 0u, 0u);         // completes the sector: no read-modify-write in DRAM
+            // streaming stores: the records are read again only by the gridding kernel, the offsets by every sample
+            if constexpr (P1) __stcs(dst, make_uint4(r.pos, r.rows, __float_as_uint(v[k].x * w[k]), __float_as_uint(v[k].y * w[k])));
+            else __stcs(dst, make_uint4(r.pos, r.rows, __float_as_uint(w[k]), (uint32_t)(first + k)));
+            __stcs(dst + 1, make_uint4(0u, 0u, 0u, 0u));   // completes the sector: no read-modify-write in DRAM
         }
     }
 }

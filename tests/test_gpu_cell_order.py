@@ -258,3 +258,43 @@ def test_dense_gcf_in_cell_order(oracle_mod, S, P, W, per_pol):
         assert_parity(grid.cpu().numpy(), ref, f"dense in cell order S={S} P={P} W={W} per_pol={per_pol}")
     finally:
         plan.destroy()
+
+
+def test_cell_order_random_shapes(oracle_mod):
+    # 30 seeded random problems: supports 3..64 (most not powers of two), 1/2/4 polarisations, oversampling 1..8,
+    # 1..5 planes, grids from the smallest the warp kernel takes, 1..60001 samples (fewer than a batch, a chunk, a
+    # warp), random walks from none to 5 cells per sample, some coordinates non-finite -- gridding (modes 1 and 2)
+    # and degridding in cell order against the oracle
+    import torch
+    from paper_1605_07023_b200 import binding
+    rng = np.random.default_rng(20260511)
+    dev = torch.device("cuda:0")
+    for it in range(30):
+        S = int(rng.choice([3, 4, 5, 7, 8, 8, 9, 12, 16, 17, 24, 32, 33, 40, 64]))
+        P = int(rng.choice([1, 2, 4]))
+        O = int(rng.choice([1, 2, 3, 4, 8]))
+        W = int(rng.choice([1, 1, 2, 5]))
+        Sk = 1 << (S - 1).bit_length()
+        N = int(rng.integers(2 * Sk + 1, max(2 * Sk + 2, 600 if S <= 16 else 300)))
+        n = int(rng.choice([1, 2, 3, 31, 33, 127, 1000, 4097, 20011, 60001]))
+        uvw, vis, wts, kernel = synth.random_problem(int(rng.integers(1 << 30)), n, N, S, O, W, P,
+                                                     spread=float(rng.choice([0.3, 0.5, 0.6])),
+                                                     walk=float(rng.choice([0.0, 0.2, 1.5, 5.0])))
+        if n > 10 and rng.random() < 0.5:
+            k = rng.integers(0, n, size=max(1, n // 50))
+            uvw[k, int(rng.integers(0, 3))] = rng.choice([np.nan, np.inf, -np.inf, 1e30])
+        what = f"case {it}: S={S} P={P} O={O} W={W} N={N} n={n}"
+        ref = oracle_mod.grid(N, S, O, W, P, uvw, vis, wts, kernel)
+        got, info = run_gpu(N, S, O, W, P, uvw, vis, wts, kernel, tuning=dict(sample_order=int(rng.choice([1, 2]))))
+        assert info["sample_order"] == 1, what
+        if np.abs(ref).max() == 0:
+            assert not got.any(), what
+        else:
+            assert_parity(got, ref, what)
+        G = (rng.standard_normal((N, N, P)) + 1j * rng.standard_normal((N, N, P))).astype(np.complex64)
+        out, _ = _gpu_degrid_cell_order(N, S, O, W, P, uvw, wts, kernel, G)
+        dref = oracle_mod.degrid(N, S, O, W, P, uvw, wts, kernel, G)
+        if np.linalg.norm(dref) == 0:
+            assert not out.any(), what
+        else:
+            assert np.linalg.norm(out - dref) <= 1e-5 * np.linalg.norm(dref), what

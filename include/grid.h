@@ -54,7 +54,9 @@ int grid_plan_set_samples(grid_plan* plan, long long n_vis);
  * never the result beyond that.  Pass zeros to clear. */
 int grid_plan_set_layout(grid_plan* plan, int n_baselines, int n_times, int n_channels);
 
-/* Scratch memory the plan needs for the current n_vis (quantised sample records + counters). */
+/* Scratch memory the plan needs for the current n_vis, layout hint and sample order (quantised sample records +
+ * counters; in cell order also the per-cell histogram and the ranks: grid_plan_set_sample_order).  Ask again after
+ * grid_plan_set_samples, grid_plan_set_layout, grid_plan_set_sample_order or grid_plan_set_tuning. */
 size_t grid_plan_workspace_bytes(const grid_plan* plan);
 /* Caller-owned device scratch, >= grid_plan_workspace_bytes(), 256-byte aligned. */
 int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes);
@@ -69,7 +71,8 @@ int grid_plan_set_workspace(grid_plan* plan, void* dev_ptr, size_t bytes);
  *   weights      [n_vis] float32
  *   conv_kernel  [n_wplanes][oversample][support] complex64 separable taps (same table for u and v)
  *   grid         [N][N][n_pol] complex64, row = v, column = u; ACCUMULATED INTO, never zeroed
- * Steps: a1 quantise pass, then the gridding kernel (a2-a9). */
+ * Steps: a1 quantise pass -- which for large inputs also sorts the samples by grid cell
+ * (grid_plan_set_sample_order) --, then the gridding kernel (a2-a9). */
 int grid_execute(grid_plan* plan, const float* uvw, const float* vis, const float* weights,
                  const float* conv_kernel, float* grid, grid_stream_t stream);
 

@@ -218,3 +218,17 @@ def test_sample_order_host_logic(binding):
         assert p.info()["sample_order"] == 0
     finally:
         p.destroy()
+
+
+def test_build_ptx_quality_check(tmp_path):
+    # __graft_entry__.build() looks at the PTX of the product library: nvcc 12.9's split compile emits, at random, a
+    # PTX that re-reads kernel parameters at every use (3.4 % slower gridding kernels); the build is repeated until the
+    # parameters are read once.  The check itself:
+    import __graft_entry__ as entry
+    good = ".visible .entry k1(\n.param .align 8 .b8 p[8])\n{\n" + "ld.param.u32 %r1, [p];\n" * 50 + "}\n"
+    (tmp_path / "gridder.ptx").write_text(good * 3)
+    assert entry._ptx_quality(str(tmp_path)) == 50
+    (tmp_path / "gridder.ptx").write_text((good + "ld.param.u64 %rd1, [p];\n" * 170) * 3)
+    q = entry._ptx_quality(str(tmp_path))
+    assert q == 220 and q > entry.LD_PARAM_PER_KERNEL >= 100
+    assert entry._ptx_quality(str(tmp_path / "missing")) is None
